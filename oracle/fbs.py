@@ -1,0 +1,180 @@
+"""Oracle: discrete energy (O3), outer forward-backward splitting loop (O5) and the
+coarse-to-fine multigrid cascade with its transfer operators (O6), in plain numpy fp64 on top
+of the C primitives.  TEST INFRASTRUCTURE — see oracle/__init__.py.
+
+Follows Algorithm A1 of the paper step by step:
+  1. g = f - (mu V / beta) dE2/df
+  2. f = argmin E1 + (beta/2) E3            (n_inner gradient-descent steps)
+  3. f = 0 where f < 0
+Readings of what the paper leaves open (Q-numbers) are listed in DESIGN.md "Readings".
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import replace
+from typing import List, Optional, Sequence
+
+import numpy as np
+
+
+def _prims():
+    import oracle as o   # the C-backed primitives
+    return o
+
+
+# ----------------------------------------------------------------------------------------
+# O3: discrete energy  (PAPER.md:65-69 with V = N_vox dV, A = N_pix du dv)
+#   E_eps(f) = (1/N_vox) sum n_ijk + mu (1/(N_theta N_pix)) sum (P f - Y)^2
+# ----------------------------------------------------------------------------------------
+def energy(g, f, Y, mu: float, eps: float, Pf: Optional[np.ndarray] = None) -> dict:
+    o = _prims()
+    if Pf is None:
+        Pf = o.forward(g, f)
+    data = float(np.sum((Pf - Y) ** 2)) / (g.n_angles * g.n_pix)
+    tv_eps = o.tv_value(g, f, eps) / g.n_vox
+    tv_0 = o.tv_value(g, f, 0.0) / g.n_vox
+    return {"E_eps": tv_eps + mu * data, "E_0": tv_0 + mu * data, "E1_eps": tv_eps, "E1_0": tv_0, "E2": data}
+
+
+# ----------------------------------------------------------------------------------------
+# O5: one level of Algorithm A1 with fixed iteration counts (Q10)
+#   c = 2 s N_vox / (N_theta N_pix),  s = step = mu/beta   (P:87 with eq. 2's factor 2; Q9)
+# ----------------------------------------------------------------------------------------
+def fbs_level(g, Y, f0, n_outer: int, n_inner: int, step: float, mu: float, eps: float,
+              omega: float = 1.0, u0_mode: str = "g", clamp: bool = True,
+              trace: Optional[list] = None) -> np.ndarray:
+    o = _prims()
+    f = np.array(f0, dtype=np.float64, copy=True)
+    beta = mu / step
+    c = 2.0 * step * g.n_vox / (g.n_angles * g.n_pix)
+    for _ in range(n_outer):
+        r = o.forward(g, f) - Y                      # P f - Y
+        G = o.backproject(g, r)                      # P^T (P f - Y)
+        gv = f - c * G                               # step 1
+        u0 = gv if u0_mode == "g" else f             # Q7: start of the inner descent
+        u = o.tv_prox(g, gv, u0, beta, eps, omega, n_inner)   # step 2
+        f = np.maximum(u, 0.0) if clamp else u       # step 3             (Q18)
+        if trace is not None:
+            trace.append(energy(g, f, Y, mu, eps))
+    return f
+
+
+# ----------------------------------------------------------------------------------------
+# O6: multigrid cascade ("multi-grid method", no details given: Q11)
+# ----------------------------------------------------------------------------------------
+def coarsen_axes(g) -> tuple:
+    """Axes (x,y,z) coarsened by 2 at the next level: those with spacing <= sqrt(2) min(h)."""
+    h = (g.hx, g.hy, g.hz)
+    m = min(h)
+    return tuple(ha <= math.sqrt(2.0) * m * (1.0 + 1e-9) for ha in h)
+
+
+def coarsen_geometry(g):
+    """Next-coarser level: halve the dims / double the spacing on coarsen_axes; bin the detector
+    2x2 (pitch doubles) iff both x and y were coarsened.  Returns (geometry, axes, binned)."""
+    ax = coarsen_axes(g)
+    n = [g.nx, g.ny, g.nz]
+    h = [g.hx, g.hy, g.hz]
+    for a in range(3):
+        if ax[a]:
+            if n[a] % 2:
+                raise ValueError("odd dimension on an axis that must coarsen")
+            n[a] //= 2
+            h[a] *= 2.0
+    binned = bool(ax[0] and ax[1])
+    nu, nv, du, dv = g.nu, g.nv, g.du, g.dv
+    if binned:
+        if nu % 2 or nv % 2:
+            raise ValueError("odd detector dimension on a level that bins the detector")
+        nu, nv, du, dv = nu // 2, nv // 2, du * 2.0, dv * 2.0
+    gc = replace(g, nu=nu, nv=nv, du=du, dv=dv, nx=n[0], ny=n[1], nz=n[2], hx=h[0], hy=h[1], hz=h[2])
+    return gc, ax, binned
+
+
+def level_geometries(g, n_levels: int):
+    """[level 0 (finest), ..., level n_levels-1 (coarsest)] with the transfer descriptors."""
+    geoms, axes, binned = [g], [], []
+    for _ in range(n_levels - 1):
+        gc, ax, b = coarsen_geometry(geoms[-1])
+        geoms.append(gc)
+        axes.append(ax)
+        binned.append(b)
+    return geoms, axes, binned
+
+
+def bin2x2(Y: np.ndarray) -> np.ndarray:
+    """Mean of each 2x2 block of detector pixels, per angle."""
+    na, nv, nu = Y.shape
+    return Y.reshape(na, nv // 2, 2, nu // 2, 2).mean(axis=(2, 4))
+
+
+def restrict_volume(f: np.ndarray, axes) -> np.ndarray:
+    """Mean over the 2 children along every coarsened axis (used only to bring a caller's f0 down)."""
+    out = f
+    for a, arr_axis in zip(range(3), (2, 1, 0)):          # x is the last array axis
+        if axes[a]:
+            sh = list(out.shape)
+            sh[arr_axis] //= 2
+            sh.insert(arr_axis + 1, 2)
+            out = out.reshape(sh).mean(axis=arr_axis + 1)
+    return out
+
+
+def _prolong_axis(c: np.ndarray, arr_axis: int) -> np.ndarray:
+    """Cell-centred linear interpolation along one array axis:
+    fine[2I] = 3/4 c[I] + 1/4 c[I-1],  fine[2I+1] = 3/4 c[I] + 1/4 c[I+1], indices clamped."""
+    c = np.moveaxis(c, arr_axis, 0)
+    n = c.shape[0]
+    lo = np.concatenate([c[:1], c[:-1]], axis=0)          # c[I-1], clamped
+    hi = np.concatenate([c[1:], c[-1:]], axis=0)          # c[I+1], clamped
+    out = np.empty((2 * n,) + c.shape[1:], dtype=c.dtype)
+    out[0::2] = 0.75 * c + 0.25 * lo
+    out[1::2] = 0.75 * c + 0.25 * hi
+    return np.moveaxis(out, 0, arr_axis)
+
+
+def prolong(c: np.ndarray, axes) -> np.ndarray:
+    """Coarse volume -> next finer level (cell-centred trilinear over the coarsened axes, x then y then z)."""
+    out = c
+    for a, arr_axis in zip(range(3), (2, 1, 0)):
+        if axes[a]:
+            out = _prolong_axis(out, arr_axis)
+    return np.ascontiguousarray(out)
+
+
+def fbs_reconstruct(g, Y, f0, n_levels: int, n_outer: Sequence[int], n_inner: int, step: float,
+                    mu: float, eps: float, omega: float = 1.0, u0_mode: str = "g",
+                    clamp: bool = True, trace: Optional[list] = None) -> np.ndarray:
+    """O6: run O5 at the coarsest level from f0 (zeros if None; a caller's fine-grid f0 is
+    restricted down), prolong to the next level, repeat; n_outer is listed coarsest first.
+    n_levels = 1 is exactly O5."""
+    assert len(n_outer) == n_levels
+    geoms, axes, binned = level_geometries(g, n_levels)
+    Ys = [np.asarray(Y, dtype=np.float64)]
+    for b in binned:
+        Ys.append(bin2x2(Ys[-1]) if b else Ys[-1])
+    if f0 is None:
+        f = np.zeros(geoms[-1].vol_shape)
+    else:
+        f = np.asarray(f0, dtype=np.float64)
+        for ax in axes:
+            f = restrict_volume(f, ax)
+    for n, lev in enumerate(range(n_levels - 1, -1, -1)):
+        f = fbs_level(geoms[lev], Ys[lev], f, n_outer[n], n_inner, step, mu, eps, omega,
+                      u0_mode=u0_mode, clamp=clamp, trace=trace)
+        if lev > 0:
+            f = prolong(f, axes[lev - 1])
+    return f
+
+
+def lambda_max(g, iters: int = 30, seed: int = 0) -> float:
+    """Largest eigenvalue of P^T P by power iteration from a seeded positive start (Q8)."""
+    o = _prims()
+    x = np.random.default_rng(seed).random(g.vol_shape) + 0.5
+    x /= np.linalg.norm(x)
+    lam = 0.0
+    for _ in range(iters):
+        y = o.backproject(g, o.forward(g, x))
+        lam = float(np.linalg.norm(y))
+        x = y / lam
+    return lam

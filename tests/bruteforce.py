@@ -1,0 +1,124 @@
+"""Independent numpy restatements used to PIN the oracle (never imported by oracle/ or by the
+CUDA path).  Everything here is the plain definition written out a second time, vectorised:
+
+* ray endpoints from the O0 convention,
+* one system-matrix entry = length of (segment S->D) ∩ (voxel box), by slab clipping,
+* smoothed isotropic TV value and its exact gradient,
+* a dense-matrix FBS iteration.
+"""
+import numpy as np
+
+
+def ray_endpoints(g):
+    """S: (na,3); D: (na,nv,nu,3)."""
+    t = np.asarray(g.angles)
+    c, s = np.cos(t), np.sin(t)
+    S = np.stack([g.sad * c, g.sad * s, np.zeros_like(t)], axis=-1)
+    uu = (np.arange(g.nu) - (g.nu - 1) / 2.0) * g.du
+    vv = (np.arange(g.nv) - (g.nv - 1) / 2.0) * g.dv
+    D = np.empty((len(t), g.nv, g.nu, 3))
+    D[..., 0] = (-(g.sdd - g.sad) * c)[:, None, None] + uu[None, None, :] * (-s)[:, None, None]
+    D[..., 1] = (-(g.sdd - g.sad) * s)[:, None, None] + uu[None, None, :] * c[:, None, None]
+    D[..., 2] = vv[None, :, None]
+    return S, D
+
+
+def clip_lengths(S, D, lo, hi):
+    """Length of segment S[r]->D[r] inside box [lo[b],hi[b]) for all (r,b): shape (R,B)."""
+    S = S[:, None, :]
+    d = (D[:, None, :] - S)
+    L = np.sqrt((d ** 2).sum(-1))
+    lo = lo[None, :, :]
+    hi = hi[None, :, :]
+    with np.errstate(divide="ignore", invalid="ignore"):
+        a0 = (lo - S) / d
+        a1 = (hi - S) / d
+    amin_a = np.minimum(a0, a1)
+    amax_a = np.maximum(a0, a1)
+    par = (d == 0.0)
+    inside = (S >= lo) & (S < hi)
+    amin_a = np.where(par, np.where(inside, -np.inf, np.inf), amin_a)
+    amax_a = np.where(par, np.where(inside, np.inf, -np.inf), amax_a)
+    amin = np.maximum(amin_a.max(-1), 0.0)
+    amax = np.minimum(amax_a.min(-1), 1.0)
+    return np.maximum(amax - amin, 0.0) * L
+
+
+def voxel_boxes(g):
+    i, j, k = np.meshgrid(np.arange(g.nx), np.arange(g.ny), np.arange(g.nz), indexing="ij")
+    # order boxes like the volume layout f[k][j][i]
+    i = i.transpose(2, 1, 0).ravel()
+    j = j.transpose(2, 1, 0).ravel()
+    k = k.transpose(2, 1, 0).ravel()
+    lo = np.stack([(i - g.nx / 2.0) * g.hx, (j - g.ny / 2.0) * g.hy, (k - g.nz / 2.0) * g.hz], -1)
+    hi = lo + np.array([g.hx, g.hy, g.hz])
+    return lo, hi
+
+
+def dense_matrix(g):
+    """(n_rays, n_vox) matrix of chord lengths, rows ordered [theta][iv][iu], columns [k][j][i]."""
+    S, D = ray_endpoints(g)
+    lo, hi = voxel_boxes(g)
+    rows = []
+    for ia in range(g.n_angles):
+        Dr = D[ia].reshape(-1, 3)
+        Sr = np.repeat(S[ia][None], Dr.shape[0], 0)
+        rows.append(clip_lengths(Sr, Dr, lo, hi))
+    return np.concatenate(rows, 0)
+
+
+def box_chords(g):
+    """P applied to the all-ones volume = length of each ray inside the volume's bounding box (pin I1)."""
+    S, D = ray_endpoints(g)
+    ext = np.array([g.nx * g.hx, g.ny * g.hy, g.nz * g.hz])
+    lo = (-ext / 2.0)[None]
+    hi = (ext / 2.0)[None]
+    out = np.empty(g.proj_shape)
+    for ia in range(g.n_angles):
+        Dr = D[ia].reshape(-1, 3)
+        Sr = np.repeat(S[ia][None], Dr.shape[0], 0)
+        out[ia] = clip_lengths(Sr, Dr, lo, hi)[:, 0].reshape(g.nv, g.nu)
+    return out
+
+
+# ---------------------------------------------------------------- TV (independent) -----
+def _diffs(f, g):
+    dx = np.zeros_like(f); dy = np.zeros_like(f); dz = np.zeros_like(f)
+    dx[:, :, :-1] = (f[:, :, 1:] - f[:, :, :-1]) / g.hx
+    dy[:, :-1, :] = (f[:, 1:, :] - f[:, :-1, :]) / g.hy
+    dz[:-1, :, :] = (f[1:, :, :] - f[:-1, :, :]) / g.hz
+    return dx, dy, dz
+
+
+def tv_value(f, g, eps):
+    dx, dy, dz = _diffs(f, g)
+    return np.sqrt(dx * dx + dy * dy + dz * dz + eps * eps).sum()   # keeps the input precision (longdouble for FD checks)
+
+
+def tv_grad(f, g, eps):
+    dx, dy, dz = _diffs(f, g)
+    n = np.sqrt(dx * dx + dy * dy + dz * dz + eps * eps)
+    px, py, pz = dx / n / g.hx, dy / n / g.hy, dz / n / g.hz
+    out = -(px + py + pz)
+    out[:, :, 1:] += px[:, :, :-1]
+    out[:, 1:, :] += py[:, :-1, :]
+    out[1:, :, :] += pz[:-1, :, :]
+    return out
+
+
+def dense_fbs(A, g, Y, f0, n_outer, n_inner, step, mu, eps, omega=1.0, u0_mode="g", clamp=True):
+    """Algorithm A1 with explicit matrix algebra; returns the list of iterates."""
+    f = f0.ravel().copy()
+    y = Y.ravel()
+    beta = mu / step
+    c = 2.0 * step * g.n_vox / (g.n_angles * g.n_pix)
+    dt = omega / (beta + 4.0 * (1 / g.hx ** 2 + 1 / g.hy ** 2 + 1 / g.hz ** 2) / eps)
+    its = []
+    for _ in range(n_outer):
+        gv = f - c * (A.T @ (A @ f - y))
+        u = (gv if u0_mode == "g" else f).copy()
+        for _ in range(n_inner):
+            u = u - dt * (beta * (u - gv) + tv_grad(u.reshape(g.vol_shape), g, eps).ravel())
+        f = np.maximum(u, 0.0) if clamp else u
+        its.append(f.reshape(g.vol_shape).copy())
+    return its
