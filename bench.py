@@ -1,0 +1,376 @@
+#!/usr/bin/env python
+"""bench.py — measurement contract of the CBCT TV-FBS hot path.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+
+Workload (N=1): BASELINE.json configs[1] ("c2"): 256^3 volume @ 1 mm, 40 views of 512x384 @ 0.78 mm.
+One STEP = one pass of the whole hot path: a 2-level coarse-to-fine
+cascade with one outer FBS iteration per level — bin Y 2x2, [P, residual, P^T, gradient step,
+10 TV-prox sweeps, clamp] on the 128^3 level, prolong, the same on the 256^3 level — through the C ABI
+call cbct_fbs_reconstruct.  Each step continues from the previous step's volume.
+metric  = projector+backprojector GUPS = voxel-projection updates of P and of P^T on all levels / step time
+value   = device-resident inputs (CUDA events around each step, L2 flushed between steps)
+e2e     = same through cbct_fbs_reconstruct_host: pinned HOST buffers, H2D of Y and f, D2H of f every step
+Extra keys: per-operator GUPS, TV GB/s, seconds per full c3 reconstruction, roofline of the dominant
+kernel (live CUDA-event timing of each kernel class), the oracle timed on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "projector+backprojector GUPS (voxel-projection updates/s of P and P^T through one full FBS cascade step)"
+UNIT = "GUPS"
+N_INNER = 10
+LEVELS = 2
+LANE_OPS_PER_CHORD = 16          # issue-bound model of the exact-chord march/gather
+NNZ = {"c2": 2.45e9, "c3": 3.85e9}   # chords per application of P; refined by frozen_params.json
+
+
+def peaks():
+    p = {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "which": "fallback"}
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            m = json.load(fh)
+        p.update(hbm_gbs=float(m["hbm_gbs"]), sm_max_mhz=float(m.get("sm_max_mhz", 1965.0)), which="measured")
+    except Exception:
+        pass
+    return p
+
+
+def frozen(key, name, default):
+    try:
+        with open(os.path.join(ROOT, "cbct_synth", "frozen_params.json")) as fh:
+            return json.load(fh).get(f"{name}/1", {}).get(key, default)
+    except Exception:
+        return default
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc:
+            time.sleep(0.25)
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for n, v in zip(names, r[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def level_dims(g, levels):
+    """(n_vox, n_rays) per level under the O6 coarsening rule (restated; no arithmetic of the method)."""
+    out = []
+    nx, ny, nz, nu, nv = g.nx, g.ny, g.nz, g.nu, g.nv
+    hx, hy, hz = g.hx, g.hy, g.hz
+    for _ in range(levels):
+        out.append((nx * ny * nz, g.n_angles * nu * nv))
+        m = min(hx, hy, hz)
+        ax = [h <= 2 ** 0.5 * m * (1 + 1e-9) for h in (hx, hy, hz)]
+        if ax[0]: nx //= 2; hx *= 2
+        if ax[1]: ny //= 2; hy *= 2
+        if ax[2]: nz //= 2; hz *= 2
+        if ax[0] and ax[1]: nu //= 2; nv //= 2
+    return out
+
+
+def run_gpu(args):
+    import torch
+    import paper_1002_3675_b200 as cb
+    from cbct_synth import make_config
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    cb.load()
+
+    cfg = make_config("c2")
+    g = cfg.geom
+    # replicas: every rank reconstructs its own independent scan (different noise-free data set per rank
+    # would be identical here, so ranks differ only by the start volume seed); no data-path collective
+    Y = np.ascontiguousarray(cfg.projections(), dtype=np.float32)
+    G = cb.Geometry.from_synth(g)
+    n_outer = [1] * LEVELS
+    lv = level_dims(g, LEVELS)
+    updates = 2.0 * sum(nvox * g.n_angles for nvox, _ in lv)
+
+    st = torch.cuda.Stream(device=dev)
+    d_Y = torch.from_numpy(Y).to(dev)
+    d_f = torch.zeros(g.vol_shape, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
+    h_Y = torch.from_numpy(Y).pin_memory()
+    h_f = torch.zeros(g.vol_shape, dtype=torch.float32).pin_memory()
+
+    def step_dev():
+        cb.fbs_reconstruct(G, d_Y, d_f, LEVELS, n_outer, N_INNER, cfg.step, cfg.mu, cfg.eps, cfg.omega, d_f, stream=st)
+
+    def step_host():
+        cb.fbs_reconstruct_host(G, h_Y, h_f, LEVELS, n_outer, N_INNER, cfg.step, cfg.mu, cfg.eps, cfg.omega, h_f, stream=st)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    with torch.cuda.stream(st):
+        for _ in range(args.warmup):
+            step_dev()
+    barrier()
+
+    # ---- timed region: K steps, device-resident, per-step events, L2 flushed between steps ----
+    cb.profile_enable(True)
+    cb.profile_read(reset=True)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    n0 = cb.launch_count()
+    with ClockSampler(local) as clk:
+        with torch.cuda.stream(st):
+            for a, b in ev:
+                flush.fill_(1)
+                a.record(st)
+                step_dev()
+                b.record(st)
+        barrier()
+    launches = cb.launch_count() - n0
+    prof = cb.profile_read(reset=True)
+    cb.profile_enable(False)
+    ms = [a.elapsed_time(b) for a, b in ev]
+    t_total = sum(ms) / 1e3
+    if dist is not None:
+        t = torch.tensor([t_total], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        t_total = float(t.item())
+
+    # ---- end-to-end: host buffers through the C ABI, copies inside the timed region ----
+    h_f.copy_(d_f.cpu())
+    with torch.cuda.stream(st):
+        step_host()                                                       # warm the staging buffers
+    barrier()
+    ev2 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    with torch.cuda.stream(st):
+        for a, b in ev2:
+            flush.fill_(1)
+            a.record(st)
+            step_host()
+            b.record(st)
+    barrier()
+    t_e2e = sum(a.elapsed_time(b) for a, b in ev2) / 1e3
+    if dist is not None:
+        t = torch.tensor([t_e2e], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        t_e2e = float(t.item())
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    pk = peaks()
+    K = args.steps
+    value = world * updates * K / t_total / 1e9
+    e2e_value = world * updates * K / t_e2e / 1e9
+
+    # per-operator numbers from the live per-class event timing (fine + coarse level launches summed)
+    def per_step_ms(tag):
+        return prof[tag][0] / K
+    upd_one = sum(nvox * g.n_angles for nvox, _ in lv)
+    gups_p = upd_one / (per_step_ms("forward") / 1e3) / 1e9
+    gups_bp = upd_one / (per_step_ms("backproject") / 1e3) / 1e9
+    tv_bytes = 12.0 * sum(nvox for nvox, _ in lv) * N_INNER
+    tv_gbs = tv_bytes / (per_step_ms("tv_sweep") / 1e3) / 1e9
+
+    # roofline of the dominant kernel class
+    dom = max(("forward", "backproject", "tv_sweep"), key=lambda t: prof[t][0])
+    nnz_fine = float(frozen("nnz", "c2", NNZ["c2"]))
+    nnz_step = nnz_fine * (1.0 + frozen("nnz_coarse_ratio", "c2", 0.125))
+    sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+    traffic = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
+            traffic = json.load(fh).get(dom)
+    except Exception:
+        pass
+    if dom == "tv_sweep":
+        roof = {"kernel": "tv_sweep_kernel", "bound": "hbm", "achieved": tv_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                "frac": tv_gbs / pk["hbm_gbs"], "traffic": traffic, "peak_source": pk["which"]}
+    else:
+        peak = sm_count * 128 * pk["sm_max_mhz"] * 1e6 / 1e12            # T lane-op/s (fp32 issue: SMs x 128 lanes x clock)
+        ach = LANE_OPS_PER_CHORD * nnz_step / (per_step_ms(dom) / 1e3) / 1e12
+        roof = {"kernel": dom + "_kernel", "bound": "alu", "achieved": ach, "peak": peak, "unit": "Tlane-op/s",
+                "frac": ach / peak, "traffic": traffic, "peak_source": pk["which"],
+                "model": f"{LANE_OPS_PER_CHORD} fp32 lane-ops per chord x {nnz_step:.3e} chords per step (SURVEY.md 8(d))",
+                "chords_per_s": nnz_step / (per_step_ms(dom) / 1e3)}
+
+    extra = {"gups_forward": gups_p, "gups_backproject": gups_bp, "tv_GBps": tv_gbs,
+             "tv_frac_of_hbm": tv_gbs / pk["hbm_gbs"],
+             "ms_per_step_by_kernel": {k: v[0] / K for k, v in prof.items()}}
+    if not args.no_recon and world == 1:
+        extra["sec_per_fbs_recon_c3"] = time_c3_recon(cb, dev, st)
+    cpu = cpu_baseline_sample(cfg, n_angles=args.cpu_angles) if world == 1 and not args.no_cpu else None
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+        "ms_per_step": 1e3 * t_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "c2: 256^3 fp32 volume @1mm, 40 views x 384x512 @0.78mm, SAD 1000/SDD 1500; "
+                               "step = 2-level FBS cascade, 1 outer iteration per level, 10 TV sweeps",
+                   "levels": LEVELS, "n_tv_inner": N_INNER, "updates_per_step": updates,
+                   "l2": "flushed between steps (256 MiB write); per-step working set ~0.9 GB > 126 MB L2",
+                   "parallelism": "replicas only (one independent reconstruction per GPU)" if world > 1 else "1 GPU"},
+        "clocks": clk.summary(),
+        "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": 1e3 * t_e2e / K,
+                "h2d_bytes_per_step": int(h_Y.numel() * 4 + h_f.numel() * 4), "d2h_bytes_per_step": int(h_f.numel() * 4)},
+        "gpu_launches": int(launches),
+        "roofline": roof,
+        "cpu_baseline": cpu,
+        "extra": extra,
+    }
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def time_c3_recon(cb, dev, st):
+    """seconds per full c3 reconstruction (2 levels x 100 outer x 10 inner; noisy 40-view data)."""
+    import torch
+    from cbct_synth import make_config
+    cfg = make_config("c3")
+    g = cfg.geom
+    Y = torch.from_numpy(np.ascontiguousarray(cfg.projections(), dtype=np.float32)).to(dev)
+    G = cb.Geometry.from_synth(g)
+    f = torch.empty(g.vol_shape, device=dev)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(st):
+        cb.fbs_reconstruct(G, Y, None, cfg.n_levels, [2] * cfg.n_levels, cfg.n_inner, cfg.step, cfg.mu, cfg.eps, cfg.omega, f, stream=st)
+        a.record(st)
+        cb.fbs_reconstruct(G, Y, None, cfg.n_levels, cfg.n_outer, cfg.n_inner, cfg.step, cfg.mu, cfg.eps, cfg.omega, f, stream=st)
+        b.record(st)
+    torch.cuda.synchronize()
+    G.close()
+    return a.elapsed_time(b) / 1e3
+
+
+def oracle_step(cfg, g, Y, f):
+    """One fine-level FBS outer iteration with the oracle as it stands."""
+    import oracle as o
+    return o.fbs_reconstruct(g, Y, f, 1, [1], N_INNER, cfg.step, cfg.mu, cfg.eps, cfg.omega)
+
+
+def cpu_baseline_sample(cfg, n_angles=8, steps=1, warmup=0):
+    """The oracle timed on this box's host cores on a bounded sample of the workload: one fine-level
+    outer iteration (P, P^T, 10 TV sweeps, clamp) of c2 restricted to `n_angles` of its 40 views."""
+    import oracle as o
+    g = cfg.geom
+    idx = np.linspace(0, g.n_angles, n_angles, endpoint=False).astype(int)
+    gs = g.with_angles(g.angles[idx])
+    Y = cfg.clean_projections(idx)
+    f = np.zeros(gs.vol_shape)
+    for _ in range(warmup):
+        f = oracle_step(cfg, gs, Y, f)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        f = oracle_step(cfg, gs, Y, f)
+    dt = (time.perf_counter() - t0) / steps
+    updates = 2.0 * gs.n_vox * gs.n_angles
+    return {"value": updates / dt / 1e9, "unit": UNIT, "cores": o.num_threads(), "kind": "oracle",
+            "seconds_per_sample_step": dt,
+            "sample": f"one fine-level FBS outer iteration (P, P^T, {N_INNER} TV sweeps, clamp) on {n_angles} of the 40 "
+                      f"views of c2 at full 256^3 volume size, fp64, OpenMP"}
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores; each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from cbct_synth import make_config
+    cfg = make_config("c2")
+    total = max(args.steps + args.warmup, 1)
+    n_angles = int(max(1, min(40, round(40 * 150.0 / (total * 45.0)))))      # ~45 s per full 40-view step on 8 cores
+    cpu = cpu_baseline_sample(cfg, n_angles=n_angles, steps=args.steps, warmup=args.warmup)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": cpu["value"], "unit": UNIT, "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * cpu["seconds_per_sample_step"],
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "c2 (bounded sample): " + cpu["sample"]},
+        "cpu_baseline": cpu,
+        "e2e": {"value": cpu["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
+    ap.add_argument("--no-recon", action="store_true", help="skip the full c3 reconstruction timing")
+    ap.add_argument("--cpu-angles", type=int, default=8)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

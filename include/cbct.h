@@ -1,0 +1,192 @@
+/*
+ * cbct.h — C ABI of libcbct.so: the B200-native (sm_100a) hot path of TV-regularised cone-beam
+ * CT reconstruction by forward-backward splitting (Jia, Lou, Li, Song, Jiang, arXiv 1002.3675).
+ *
+ * Citations: P:<n> = PAPER.md line n (the paper); O<n>/Q<n> = the readings in DESIGN.md
+ * (the paper leaves the discretisation open; every choice is listed there).
+ *
+ * Conventions (all entry points)
+ *   - Lengths in mm, angles in radians.  Rotation axis z.  Source S(t) = (SAD cos t, SAD sin t, 0);
+ *     detector centre -(SDD-SAD)(cos t, sin t, 0); detector axes u^ = (-sin t, cos t, 0), v^ = z^;
+ *     pixel (iu,iv) centre at ((iu-(nu-1)/2) du, (iv-(nv-1)/2) dv); volume centred at the origin.
+ *   - Volume layout   f[k][j][i]  (x fastest), nz*ny*nx floats.
+ *     Projection layout Y[a][iv][iu] (u fastest), n_angles*nv*nu floats.
+ *   - Pointers named d_* are DEVICE pointers to contiguous fp32 memory owned by the caller
+ *     (e.g. a PyTorch CUDA tensor); pointers named h_* are HOST pointers.  The library never frees
+ *     or reallocates caller memory.  Inputs and outputs must not alias unless stated.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device
+ *     entry points are asynchronous on that stream; they synchronise with the host only where
+ *     stated.  The *_host entry points copy host<->device on that stream and return after
+ *     synchronising it.
+ *   - A handle owns per-angle ray tables and lazily allocated scratch (grown on first use, freed
+ *     by cbct_geometry_destroy).  A handle must not be used from two host threads or two streams
+ *     at the same time.
+ *   - Errors: every call returns a cbct_status; nothing throws or aborts across the ABI.  On
+ *     failure outputs are unspecified and cbct_last_error() describes the failure (thread-local).
+ *   - There is no CPU fallback: with no CUDA device every compute call returns CBCT_ERR_CUDA.
+ */
+#ifndef CBCT_H
+#define CBCT_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cbct_geometry cbct_geometry;   /* opaque, library-owned */
+
+typedef enum {
+    CBCT_OK = 0,
+    CBCT_ERR_INVALID_ARG = 1,   /* NULL required pointer, non-positive size or parameter */
+    CBCT_ERR_SHAPE = 2,         /* geometry the kernels do not support (see cbct_geometry_create), odd
+                                   dimension on an axis that must coarsen */
+    CBCT_ERR_ALLOC = 3,         /* host or device allocation failed */
+    CBCT_ERR_CUDA = 4           /* a CUDA runtime call or kernel launch failed, or no device */
+} cbct_status;
+
+/*
+ * Scan geometry ("an operator P^theta projects f onto an x-ray imager plane in a cone beam
+ * geometry at an angle theta"; convention O0).
+ *   sad_mm, sdd_mm     source-axis and source-detector distance (L0 of P:99); 0 < sad < sdd
+ *   h_angles_rad       HOST array of n_angles projection angles, any list (360 deg equi-spaced P:119,
+ *                      200 deg arc P:121); copied
+ *   nu, nv, du, dv     detector pixels and pitch ("512 x 384 detectors" = nu x nv)
+ *   nx..nz, hx..hz     volume dims and voxel size
+ * Builds the per-(angle,u) ray tables (fp64 on the host, stored fp32 on the device).
+ * Errors: INVALID_ARG for NULL / non-positive values or sad >= sdd; SHAPE if the volume's
+ * circumscribed cylinder is not strictly between source and detector, if a dimension exceeds
+ * 16384, or if some ray climbs more than 0.999 voxels in z per voxel of its major (x or y) axis
+ * (the slab march assumes at most one z-plane crossing per slab; true for every cone-beam CT
+ * geometry with hz not much smaller than hx, hy).  No device memory is touched if this fails.
+ */
+cbct_status cbct_geometry_create(double sad_mm, double sdd_mm,
+                                 const double *h_angles_rad, int n_angles,
+                                 int nu, int nv, double du_mm, double dv_mm,
+                                 int nx, int ny, int nz, double hx_mm, double hy_mm, double hz_mm,
+                                 cbct_geometry **out);
+
+/* Frees the handle, its coarse-level handles and all scratch.  NULL is allowed.  Synchronises the device. */
+void cbct_geometry_destroy(cbct_geometry *g);
+
+/* Writes {n_angles, nu, nv, nx, ny, nz} to h_dims6 and {du, dv, hx, hy, hz} to h_sizes5 (either may be NULL). */
+cbct_status cbct_geometry_query(const cbct_geometry *g, int *h_dims6, double *h_sizes5);
+
+/*
+ * Next-coarser multigrid level ("multi-grid method"; reading O6/Q11): every axis whose spacing
+ * is <= sqrt(2) * min(hx,hy,hz) is coarsened by 2 (dims halve, spacing doubles); the detector is
+ * binned 2x2 (pitch doubles) iff both x and y were coarsened.  The returned handle is OWNED BY `g`
+ * (freed with it; repeated calls return the same handle).  h_flags4 (may be NULL) receives
+ * {x coarsened, y coarsened, z coarsened, detector binned}.
+ * Errors: SHAPE for an odd dimension on an axis that must coarsen (or odd nu/nv when binning).
+ */
+cbct_status cbct_geometry_coarsen(const cbct_geometry *g, cbct_geometry **out_coarse, int *h_flags4);
+
+/*
+ * a1. Forward projection q = P f (definition O1): for every angle and detector pixel,
+ * the sum over voxels of (length of the segment source->pixel-centre inside the voxel box) * f.
+ * Rays that miss the volume give 0.  d_proj is overwritten.
+ */
+cbct_status cbct_forward(const cbct_geometry *g, const float *d_vol, float *d_proj, void *cuda_stream);
+
+/*
+ * a3. Backprojection G = P^T y — the exact transpose of cbct_forward's matrix ("P^T denotes a
+ * matrix transpose"; O2), evaluated as a race-free gather (the paper's "memory conflict" remark,
+ * P:95): <P x, y> = <x, P^T y> up to fp32 rounding.  d_vol is overwritten.
+ */
+cbct_status cbct_backproject(const cbct_geometry *g, const float *d_proj, float *d_vol, void *cuda_stream);
+
+/*
+ * a5. TV-prox inner descent (P:89 step 2, "solved by a simple gradient descent method"; O4):
+ * n_inner Jacobi steps  u <- u - dt [ beta (u - g) + grad TV_eps(u) ],
+ *   dt = omega / (beta + 4 (1/hx^2 + 1/hy^2 + 1/hz^2) / eps),
+ * TV_eps = sum sqrt(dx^2+dy^2+dz^2+eps^2) with forward differences divided by the spacing, zero at
+ * the far faces.  d_u holds the start on entry and the result on exit (d_u == d_g is NOT allowed;
+ * copy g into u to start from g).  Only the volume dims / voxel sizes of `g` are used.
+ * Errors: INVALID_ARG if beta < 0, eps <= 0, omega <= 0 or n_inner < 0.
+ */
+cbct_status cbct_tv_prox(const cbct_geometry *g, const float *d_g, float *d_u,
+                         float beta, float eps, float omega, int n_inner, void *cuda_stream);
+
+/*
+ * a7. Multigrid transfers between `fine` and its coarse level (cbct_geometry_coarsen(fine)); O6.
+ *   cbct_prolong : coarse volume -> fine volume, cell-centred linear interpolation along every
+ *                  coarsened axis (fine 2I = 3/4 c[I] + 1/4 c[I-1], fine 2I+1 = 3/4 c[I] + 1/4 c[I+1],
+ *                  indices clamped), copy along the others.
+ *   cbct_restrict: fine volume -> coarse volume, mean of the children (used for a caller's f0).
+ *   cbct_bin2x2  : fine projections -> coarse projections, mean of each 2x2 pixel block (plain
+ *                  copy if the level does not bin the detector).
+ */
+cbct_status cbct_prolong (const cbct_geometry *fine, const float *d_coarse_vol, float *d_fine_vol, void *cuda_stream);
+cbct_status cbct_restrict(const cbct_geometry *fine, const float *d_fine_vol, float *d_coarse_vol, void *cuda_stream);
+cbct_status cbct_bin2x2  (const cbct_geometry *fine, const float *d_fine_proj, float *d_coarse_proj, void *cuda_stream);
+
+/*
+ * Discrete energy of eq. 1 (O3):
+ *   E_eps(f) = (1/N_vox) sum n_ijk + mu (1/(N_theta N_pix)) sum (P f - Y)^2 .
+ * h_out3 receives {E_eps, E1_eps = TV_eps/N_vox, E2 = data term without mu} as doubles.
+ * Runs a forward projection and deterministic two-stage reductions; SYNCHRONISES the stream.
+ */
+cbct_status cbct_energy(const cbct_geometry *g, const float *d_f, const float *d_Y,
+                        float mu, float eps, double *h_out3, void *cuda_stream);
+
+/*
+ * The hot path: Algorithm A1 inside a coarse-to-fine cascade (O5/O6).
+ * For level l = n_levels-1 (coarsest) ... 0 (finest = g), n_outer_per_level[] listed COARSEST FIRST:
+ *   repeat n_outer times:
+ *     r = P f - Y                     (a1 + a2, fused)
+ *     G = P^T r                       (a3)
+ *     gv = f - c G, c = 2 step N_vox / (N_theta N_pix)      (a4; P:87 with eq. 2's factor 2)
+ *     u = gv; n_tv_inner TV-prox steps with beta = mu / step  (a5)
+ *     f = max(u, 0)                   (a6)
+ *   prolong f to the next finer level (a7).
+ * Y for the coarse levels is the 2x2-binned d_Y.  d_f0 == NULL starts from zeros; otherwise d_f0 is
+ * a FINEST-level volume that is restricted down to the coarsest level.  n_levels == 1 is plain A1.
+ * d_f_out (finest level) is overwritten; it may equal d_f0.
+ * h_energy_trace: NULL, or sum(n_outer_per_level) doubles receiving E_eps after every outer
+ * iteration (costs one extra forward projection and a stream synchronise per iteration).
+ * Without a trace the call is asynchronous.
+ * Errors: INVALID_ARG for n_levels < 1, negative counts, step <= 0, mu <= 0, eps <= 0, omega <= 0;
+ * SHAPE as for cbct_geometry_coarsen.
+ */
+cbct_status cbct_fbs_reconstruct(const cbct_geometry *g, const float *d_Y, const float *d_f0,
+                                 int n_levels, const int *n_outer_per_level, int n_tv_inner,
+                                 float step, float mu, float eps, float omega,
+                                 float *d_f_out, double *h_energy_trace, void *cuda_stream);
+
+/*
+ * Host-buffer variants (end-to-end path): same operations with HOST pointers; each call copies its
+ * inputs host->device and its result device->host on `cuda_stream` (use pinned host memory for
+ * full copy speed) and returns after synchronising the stream.
+ */
+cbct_status cbct_forward_host(const cbct_geometry *g, const float *h_vol, float *h_proj, void *cuda_stream);
+cbct_status cbct_backproject_host(const cbct_geometry *g, const float *h_proj, float *h_vol, void *cuda_stream);
+cbct_status cbct_tv_prox_host(const cbct_geometry *g, const float *h_g, float *h_u,
+                              float beta, float eps, float omega, int n_inner, void *cuda_stream);
+cbct_status cbct_fbs_reconstruct_host(const cbct_geometry *g, const float *h_Y, const float *h_f0,
+                                      int n_levels, const int *n_outer_per_level, int n_tv_inner,
+                                      float step, float mu, float eps, float omega,
+                                      float *h_f_out, double *h_energy_trace, void *cuda_stream);
+
+/*
+ * Per-kernel-class device timing (CUDA events recorded around each launch on the launching stream).
+ * Classes: 0 pad/transposed volume copies, 1 forward projector, 2 projection scaling, 3 backprojector
+ * gather, 4 combine / gradient step, 5 TV sweep, 6 multigrid transfers, 7 reductions.
+ * cbct_profile_read fills h_ms[CBCT_PROFILE_TAGS] (summed milliseconds) and h_count[] (launch groups)
+ * since the last reset; it waits for the recorded events.  Off by default.
+ */
+#define CBCT_PROFILE_TAGS 8
+cbct_status cbct_profile_enable(int on);
+cbct_status cbct_profile_read(double *h_ms, unsigned long long *h_count, int reset);
+
+/* Number of kernels this library has launched in this process so far (monotone counter). */
+unsigned long long cbct_launch_count(void);
+
+/* Bytes of device memory currently held by the handle (tables + scratch, all levels). */
+unsigned long long cbct_device_bytes(const cbct_geometry *g);
+
+/* Description of the last failure on this host thread ("" if none).  Static storage. */
+const char *cbct_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CBCT_H */

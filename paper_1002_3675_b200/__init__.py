@@ -1,0 +1,14 @@
+"""paper_1002_3675_b200 — B200-native (sm_100a) hot path of TV-regularised cone-beam CT
+reconstruction by forward-backward splitting (arXiv 1002.3675).
+
+Thin Python binding over the C ABI of `libcbct.so` (include/cbct.h): argument marshalling only —
+every step of the path runs in the hand-written CUDA kernels under `csrc/`.  PyTorch supplies
+device memory and streams.  There is no CPU fallback: loading fails loudly if the library is
+missing, and every compute call fails if there is no CUDA device.
+"""
+from .binding import (  # noqa: F401
+    CbctError, Geometry, load, lib_path, launch_count,
+    forward, backproject, tv_prox, fbs_reconstruct, energy, prolong, restrict, bin2x2,
+    profile_enable, profile_read, PROFILE_TAGS,
+    forward_host, backproject_host, tv_prox_host, fbs_reconstruct_host,
+)

@@ -1,0 +1,263 @@
+// C-ABI entry points (include/cbct.h): argument checks, scratch, the FBS / multigrid driver (L2) and
+// the host-buffer variants.  All arithmetic of the hot path runs in the kernels of projector.cu,
+// backprojector.cu, tv.cu and transfers.cu.
+#include <cmath>
+#include <vector>
+
+#include "cbct_internal.h"
+
+#define REQUIRE(cond, ...)                                  \
+    do {                                                    \
+        if (!(cond)) {                                      \
+            cbct_set_error(__VA_ARGS__);                    \
+            return CBCT_ERR_INVALID_ARG;                    \
+        }                                                   \
+    } while (0)
+
+static inline cbct_geometry *mut(const cbct_geometry *g) { return const_cast<cbct_geometry *>(g); }
+
+extern "C" cbct_status cbct_forward(const cbct_geometry *gc, const float *d_vol, float *d_proj, void *stream)
+{
+    REQUIRE(gc && d_vol && d_proj, "cbct_forward: NULL argument");
+    cbct_geometry *g = mut(gc);
+    cudaStream_t st = (cudaStream_t)stream;
+    CBCT_TRY(op_pad_copies(g, d_vol, st));
+    return op_forward_padded(g, d_proj, nullptr, 0, st);
+}
+
+extern "C" cbct_status cbct_backproject(const cbct_geometry *gc, const float *d_proj, float *d_vol, void *stream)
+{
+    REQUIRE(gc && d_proj && d_vol, "cbct_backproject: NULL argument");
+    cbct_geometry *g = mut(gc);
+    cudaStream_t st = (cudaStream_t)stream;
+    CBCT_TRY(ensure(g, &g->proj_tmp, g->n_proj(), true));
+    CBCT_TRY(op_scale_proj(g, d_proj, g->proj_tmp, st));
+    CBCT_TRY(op_backproject_gather(g, g->proj_tmp, st));
+    return op_combine(g, nullptr, 0.f, 0, d_vol, st);
+}
+
+static float tv_dt(const cbct_geometry *g, float beta, float eps, float omega)
+{
+    const double K = 4.0 * (1.0 / (g->hx * g->hx) + 1.0 / (g->hy * g->hy) + 1.0 / (g->hz * g->hz));
+    return (float)((double)omega / ((double)beta + K / (double)eps));
+}
+
+// n_inner Jacobi steps starting from u_start (may alias gv or u_out); the result ends in u_out.
+// vol_b is the second ping-pong buffer.  clamp_last fuses a6 into the last step's store.
+static cbct_status tv_inner(cbct_geometry *g, const float *gv, const float *u_start, float *u_out, float beta,
+                            float eps, float omega, int n_inner, int clamp_last, cudaStream_t st)
+{
+    const size_t bytes = g->n_vox() * sizeof(float);
+    if (n_inner == 0) {
+        if (u_start != u_out) CBCT_CUDA(cudaMemcpyAsync(u_out, u_start, bytes, cudaMemcpyDeviceToDevice, st));
+        return CBCT_OK;
+    }
+    CBCT_TRY(ensure(g, &g->vol_b, g->n_vox()));
+    const float dt = tv_dt(g, beta, eps, omega);
+    const float *src = u_start;
+    for (int m = 0; m < n_inner; ++m) {
+        float *dst = ((n_inner - 1 - m) % 2 == 0) ? u_out : g->vol_b;     // the last step lands in u_out
+        if (src == dst) {                                                  // only m == 0 with u_start == u_out
+            CBCT_CUDA(cudaMemcpyAsync(g->vol_b, src, bytes, cudaMemcpyDeviceToDevice, st));
+            src = g->vol_b;
+        }
+        CBCT_TRY(op_tv_sweep(g, src, gv, dst, beta, eps, dt, clamp_last && m == n_inner - 1, st));
+        src = dst;
+    }
+    return CBCT_OK;
+}
+
+extern "C" cbct_status cbct_tv_prox(const cbct_geometry *gc, const float *d_g, float *d_u, float beta, float eps,
+                                    float omega, int n_inner, void *stream)
+{
+    REQUIRE(gc && d_g && d_u, "cbct_tv_prox: NULL argument");
+    REQUIRE(d_g != d_u, "cbct_tv_prox: d_u must not alias d_g");
+    REQUIRE(beta >= 0.f && eps > 0.f && omega > 0.f && n_inner >= 0, "cbct_tv_prox: beta < 0, eps <= 0, omega <= 0 or n_inner < 0");
+    return tv_inner(mut(gc), d_g, d_u, d_u, beta, eps, omega, n_inner, 0, (cudaStream_t)stream);
+}
+
+extern "C" cbct_status cbct_prolong(const cbct_geometry *fine, const float *c, float *f, void *stream)
+{
+    REQUIRE(fine && c && f, "cbct_prolong: NULL argument");
+    return op_prolong(mut(fine), c, f, (cudaStream_t)stream);
+}
+extern "C" cbct_status cbct_restrict(const cbct_geometry *fine, const float *f, float *c, void *stream)
+{
+    REQUIRE(fine && c && f, "cbct_restrict: NULL argument");
+    return op_restrict(mut(fine), f, c, (cudaStream_t)stream);
+}
+extern "C" cbct_status cbct_bin2x2(const cbct_geometry *fine, const float *y, float *yc, void *stream)
+{
+    REQUIRE(fine && y && yc, "cbct_bin2x2: NULL argument");
+    return op_bin2x2(mut(fine), y, yc, (cudaStream_t)stream);
+}
+
+// E_eps(f); synchronises.
+static cbct_status energy_impl(cbct_geometry *g, const float *d_f, const float *d_Y, float mu, float eps,
+                               double *out3, cudaStream_t st)
+{
+    CBCT_TRY(ensure(g, &g->proj_tmp, g->n_proj(), true));
+    CBCT_TRY(ensure(g, &g->red_out, (size_t)2));
+    if (!g->h_red) CBCT_CUDA(cudaMallocHost((void **)&g->h_red, 2 * sizeof(double)));
+    CBCT_TRY(op_pad_copies(g, d_f, st));
+    CBCT_TRY(op_forward_padded(g, g->proj_tmp, nullptr, 0, st));
+    CBCT_TRY(op_sumsq_diff(g, g->proj_tmp, d_Y, g->n_proj(), g->red_out + 0, st));
+    CBCT_TRY(op_tv_value(g, d_f, eps, g->red_out + 1, st));
+    CBCT_CUDA(cudaMemcpyAsync(g->h_red, g->red_out, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CBCT_CUDA(cudaStreamSynchronize(st));
+    const double e2 = g->h_red[0] / ((double)g->na * g->nu * g->nv);
+    const double e1 = g->h_red[1] / (double)g->n_vox();
+    out3[0] = e1 + (double)mu * e2;
+    out3[1] = e1;
+    out3[2] = e2;
+    return CBCT_OK;
+}
+
+extern "C" cbct_status cbct_energy(const cbct_geometry *gc, const float *d_f, const float *d_Y, float mu, float eps,
+                                   double *h_out3, void *stream)
+{
+    REQUIRE(gc && d_f && d_Y && h_out3, "cbct_energy: NULL argument");
+    REQUIRE(eps >= 0.f, "cbct_energy: eps < 0");
+    return energy_impl(mut(gc), d_f, d_Y, mu, eps, h_out3, (cudaStream_t)stream);
+}
+
+// One level of Algorithm A1: f (in/out, level-sized device buffer).
+static cbct_status fbs_level(cbct_geometry *g, const float *d_Y, float *f, int n_outer, int n_inner, float step,
+                             float mu, float eps, float omega, double *trace, cudaStream_t st)
+{
+    CBCT_TRY(ensure(g, &g->proj_tmp, g->n_proj(), true));
+    CBCT_TRY(ensure(g, &g->vol_a, g->n_vox()));
+    const float beta = mu / step;
+    const float c = (float)(2.0 * (double)step * (double)g->n_vox() / ((double)g->na * g->nu * g->nv));
+    for (int it = 0; it < n_outer; ++it) {
+        CBCT_TRY(op_pad_copies(g, f, st));
+        CBCT_TRY(op_forward_padded(g, g->proj_tmp, d_Y, 1, st));          // l (P f - Y)          a1+a2
+        CBCT_TRY(op_backproject_gather(g, g->proj_tmp, st));              // P^T (P f - Y)        a3
+        if (n_inner == 0) {
+            CBCT_TRY(op_combine(g, f, c, 1, g->vol_a, st));               // max(f - c G, 0)      a4+a6
+            CBCT_CUDA(cudaMemcpyAsync(f, g->vol_a, g->n_vox() * sizeof(float), cudaMemcpyDeviceToDevice, st));
+        } else {
+            CBCT_TRY(op_combine(g, f, c, 0, g->vol_a, st));               // gv = f - c G         a4
+            CBCT_TRY(tv_inner(g, g->vol_a, g->vol_a, f, beta, eps, omega, n_inner, 1, st));   // u0 = gv (Q7); a5 + a6
+        }
+        if (trace) {
+            double e3[3];
+            CBCT_TRY(energy_impl(g, f, d_Y, mu, eps, e3, st));
+            trace[it] = e3[0];
+        }
+    }
+    return CBCT_OK;
+}
+
+extern "C" cbct_status cbct_fbs_reconstruct(const cbct_geometry *gc, const float *d_Y, const float *d_f0, int n_levels,
+                                            const int *n_outer, int n_inner, float step, float mu, float eps,
+                                            float omega, float *d_f_out, double *trace, void *stream)
+{
+    REQUIRE(gc && d_Y && d_f_out && n_outer, "cbct_fbs_reconstruct: NULL argument");
+    REQUIRE(n_levels >= 1 && n_levels <= 16 && n_inner >= 0, "cbct_fbs_reconstruct: n_levels < 1 (or > 16) or n_tv_inner < 0");
+    REQUIRE(step > 0.f && mu > 0.f && eps > 0.f && omega > 0.f, "cbct_fbs_reconstruct: step, mu, eps and omega must be > 0");
+    for (int l = 0; l < n_levels; ++l) REQUIRE(n_outer[l] >= 0, "cbct_fbs_reconstruct: negative iteration count");
+    cudaStream_t st = (cudaStream_t)stream;
+
+    // level handles, finest first
+    std::vector<cbct_geometry *> lev(n_levels);
+    lev[0] = mut(gc);
+    for (int l = 1; l < n_levels; ++l) CBCT_TRY(cbct_geometry_coarsen(lev[l - 1], &lev[l], nullptr));
+
+    // data per level: level 0 uses d_Y, coarser levels their own binned copy
+    std::vector<const float *> Y(n_levels);
+    Y[0] = d_Y;
+    for (int l = 1; l < n_levels; ++l) {
+        CBCT_TRY(ensure(lev[l], &lev[l]->Y_level, lev[l]->n_proj()));
+        CBCT_TRY(op_bin2x2(lev[l - 1], Y[l - 1], lev[l]->Y_level, st));
+        Y[l] = lev[l]->Y_level;
+    }
+    // current iterate per level lives in vol_f of that level (level 0: the caller's output buffer)
+    std::vector<float *> F(n_levels);
+    F[0] = d_f_out;
+    for (int l = 1; l < n_levels; ++l) {
+        CBCT_TRY(ensure(lev[l], &lev[l]->vol_f, lev[l]->n_vox()));
+        F[l] = lev[l]->vol_f;
+    }
+    // start: zeros, or the caller's fine f0 restricted down
+    const int L = n_levels - 1;
+    if (!d_f0) {
+        CBCT_CUDA(cudaMemsetAsync(F[L], 0, lev[L]->n_vox() * sizeof(float), st));
+    } else {
+        if (d_f0 != d_f_out)
+            CBCT_CUDA(cudaMemcpyAsync(F[0], d_f0, lev[0]->n_vox() * sizeof(float), cudaMemcpyDeviceToDevice, st));
+        for (int l = 1; l < n_levels; ++l) CBCT_TRY(op_restrict(lev[l - 1], F[l - 1], F[l], st));
+    }
+    int done = 0;
+    for (int l = L; l >= 0; --l) {
+        const int n = n_outer[L - l];
+        CBCT_TRY(fbs_level(lev[l], Y[l], F[l], n, n_inner, step, mu, eps, omega, trace ? trace + done : nullptr, st));
+        done += n;
+        if (l > 0) CBCT_TRY(op_prolong(lev[l - 1], F[l], F[l - 1], st));
+    }
+    return CBCT_OK;
+}
+
+// ---- host-buffer variants ----------------------------------------------------------------------
+extern "C" cbct_status cbct_forward_host(const cbct_geometry *gc, const float *h_vol, float *h_proj, void *stream)
+{
+    REQUIRE(gc && h_vol && h_proj, "cbct_forward_host: NULL argument");
+    cbct_geometry *g = mut(gc);
+    cudaStream_t st = (cudaStream_t)stream;
+    CBCT_TRY(ensure(g, &g->host_stage_vol, g->n_vox()));
+    CBCT_TRY(ensure(g, &g->host_stage_proj, g->n_proj()));
+    CBCT_CUDA(cudaMemcpyAsync(g->host_stage_vol, h_vol, g->n_vox() * sizeof(float), cudaMemcpyHostToDevice, st));
+    CBCT_TRY(cbct_forward(g, g->host_stage_vol, g->host_stage_proj, stream));
+    CBCT_CUDA(cudaMemcpyAsync(h_proj, g->host_stage_proj, g->n_proj() * sizeof(float), cudaMemcpyDeviceToHost, st));
+    CBCT_CUDA(cudaStreamSynchronize(st));
+    return CBCT_OK;
+}
+
+extern "C" cbct_status cbct_backproject_host(const cbct_geometry *gc, const float *h_proj, float *h_vol, void *stream)
+{
+    REQUIRE(gc && h_vol && h_proj, "cbct_backproject_host: NULL argument");
+    cbct_geometry *g = mut(gc);
+    cudaStream_t st = (cudaStream_t)stream;
+    CBCT_TRY(ensure(g, &g->host_stage_vol, g->n_vox()));
+    CBCT_TRY(ensure(g, &g->host_stage_proj, g->n_proj()));
+    CBCT_CUDA(cudaMemcpyAsync(g->host_stage_proj, h_proj, g->n_proj() * sizeof(float), cudaMemcpyHostToDevice, st));
+    CBCT_TRY(cbct_backproject(g, g->host_stage_proj, g->host_stage_vol, stream));
+    CBCT_CUDA(cudaMemcpyAsync(h_vol, g->host_stage_vol, g->n_vox() * sizeof(float), cudaMemcpyDeviceToHost, st));
+    CBCT_CUDA(cudaStreamSynchronize(st));
+    return CBCT_OK;
+}
+
+extern "C" cbct_status cbct_tv_prox_host(const cbct_geometry *gc, const float *h_g, float *h_u, float beta, float eps,
+                                         float omega, int n_inner, void *stream)
+{
+    REQUIRE(gc && h_g && h_u, "cbct_tv_prox_host: NULL argument");
+    cbct_geometry *g = mut(gc);
+    cudaStream_t st = (cudaStream_t)stream;
+    CBCT_TRY(ensure(g, &g->host_stage_vol, g->n_vox()));
+    CBCT_TRY(ensure(g, &g->host_stage_vol2, g->n_vox()));
+    CBCT_CUDA(cudaMemcpyAsync(g->host_stage_vol, h_g, g->n_vox() * sizeof(float), cudaMemcpyHostToDevice, st));
+    CBCT_CUDA(cudaMemcpyAsync(g->host_stage_vol2, h_u, g->n_vox() * sizeof(float), cudaMemcpyHostToDevice, st));
+    CBCT_TRY(cbct_tv_prox(g, g->host_stage_vol, g->host_stage_vol2, beta, eps, omega, n_inner, stream));
+    CBCT_CUDA(cudaMemcpyAsync(h_u, g->host_stage_vol2, g->n_vox() * sizeof(float), cudaMemcpyDeviceToHost, st));
+    CBCT_CUDA(cudaStreamSynchronize(st));
+    return CBCT_OK;
+}
+
+extern "C" cbct_status cbct_fbs_reconstruct_host(const cbct_geometry *gc, const float *h_Y, const float *h_f0,
+                                                 int n_levels, const int *n_outer, int n_inner, float step, float mu,
+                                                 float eps, float omega, float *h_f_out, double *trace, void *stream)
+{
+    REQUIRE(gc && h_Y && h_f_out, "cbct_fbs_reconstruct_host: NULL argument");
+    cbct_geometry *g = mut(gc);
+    cudaStream_t st = (cudaStream_t)stream;
+    CBCT_TRY(ensure(g, &g->host_stage_vol, g->n_vox()));
+    CBCT_TRY(ensure(g, &g->host_stage_proj, g->n_proj()));
+    CBCT_CUDA(cudaMemcpyAsync(g->host_stage_proj, h_Y, g->n_proj() * sizeof(float), cudaMemcpyHostToDevice, st));
+    if (h_f0)
+        CBCT_CUDA(cudaMemcpyAsync(g->host_stage_vol, h_f0, g->n_vox() * sizeof(float), cudaMemcpyHostToDevice, st));
+    CBCT_TRY(cbct_fbs_reconstruct(g, g->host_stage_proj, h_f0 ? g->host_stage_vol : nullptr, n_levels, n_outer, n_inner,
+                                  step, mu, eps, omega, g->host_stage_vol, trace, stream));
+    CBCT_CUDA(cudaMemcpyAsync(h_f_out, g->host_stage_vol, g->n_vox() * sizeof(float), cudaMemcpyDeviceToHost, st));
+    CBCT_CUDA(cudaStreamSynchronize(st));
+    return CBCT_OK;
+}

@@ -1,0 +1,164 @@
+// Internal declarations of libcbct (CUDA path).  Not part of the ABI; see include/cbct.h.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <cstdio>
+#include <vector>
+
+#include "../../include/cbct.h"
+
+// ------------------------------------------------------------------------------------------
+// Device-side geometry.  Every ray is traversed slab by slab along its MAJOR axis: x if
+// |dX| >= |dY| in voxel units (class 0), else y (class 1); the other in-plane axis is MINOR.
+// |d minor / d major| <= 1 by construction, so a ray crosses at most one minor plane per slab.
+// ------------------------------------------------------------------------------------------
+constexpr int kPadLo = 4;      // zero floats before minor index 0 in the padded copies (>= 2; 4 keeps rows 16-B aligned)
+constexpr int kPadHi = 2;      // zero floats after minor index nmin-1 (>= 2)
+constexpr int kPadK = 2;       // zero planes below k = 0 and above k = nz-1
+
+// Per-(angle,u) constants, computed in fp64 on the host.  32 bytes = two 16-byte loads.
+struct __align__(16) RayXY {
+    float mc;       // minor coordinate (voxel units, minus joff) where the ray meets major plane ioff
+    float sm;       // d(minor)/d(major), voxel units
+    float inv_sm;   // 1/sm (+1e30 if sm == 0)
+    float tc;       // ray parameter t in [0,1] at major plane ioff
+    float dt;       // dt per major voxel (signed)
+    float inv_dt;   // 1/dt
+    float lxy2;     // hmaj^2 + (sm hmin)^2  [mm^2]; chord per slab = sqrt(lxy2 + (dt Dz)^2)
+    int range;      // bits 0-14 ilo, 15-29 ihi (slabs where the ray can touch minor range [-1,nmin+1]), bit 30 class
+};
+__host__ __device__ inline int ray_ilo(int r) { return r & 0x7fff; }
+__host__ __device__ inline int ray_ihi(int r) { return (r >> 15) & 0x7fff; }
+__host__ __device__ inline int ray_cls(int r) { return (r >> 30) & 1; }
+
+// Per-class view of the volume grid (class 0: major x / minor y; class 1: major y / minor x).
+struct ClassGrid {
+    int nmaj, nmin, ioff, joff;
+    float hmaj, hmin;
+    int row_stride;             // floats per padded minor row
+    long long plane_stride;     // floats per padded k-plane = nmaj * row_stride
+};
+
+struct DevGeom {
+    int na, nu, nv, nx, ny, nz;
+    int koff;                   // nz / 2
+    float zfrac;                // nz/2.0 - koff  (0 or 0.5)
+    float hx, hy, hz, du, dv, sad, sdd;
+    ClassGrid cls[2];
+    const RayXY *rays;          // [na][nu]
+    const float *zeta;          // [nv]  Dz(v)/hz
+    const float *inv_zeta;      // [nv]  hz/Dz(v) (+-1e30 if Dz == 0)
+    const float *dz_mm;         // [nv]  Dz(v) in mm
+    const float2 *cs;           // [na]  (cos, sin)
+};
+
+// Host-side handle.
+struct cbct_geometry {
+    // user geometry (fp64)
+    double sad, sdd, du, dv, hx, hy, hz;
+    int na, nu, nv, nx, ny, nz;
+    std::vector<double> angles;
+
+    DevGeom dev{};
+    // device tables
+    RayXY *d_rays = nullptr;
+    float *d_zeta = nullptr, *d_inv_zeta = nullptr, *d_dz = nullptr;
+    float2 *d_cs = nullptr;
+    int2 *d_tiles[2] = {nullptr, nullptr};   // forward work list per class: (angle, u0)
+    int n_tiles[2] = {0, 0};
+    unsigned char *d_angle_has[2] = {nullptr, nullptr};   // [na] does this angle have rays of the class
+    std::vector<unsigned char> h_angle_has[2];
+    float max_abs_sz = 0.f;
+
+    // lazily allocated scratch (device)
+    float *vol_pad[2] = {nullptr, nullptr};   // padded [nz+2K][nmaj][row_stride] copies (class 0 transposed)
+    float *proj_tmp = nullptr;                // scaled residual / projections
+    float *G_cls[2] = {nullptr, nullptr};     // per-class backprojection outputs (class 0 in [k][i][j] order)
+    float *vol_a = nullptr, *vol_b = nullptr, *vol_c = nullptr, *vol_f = nullptr;   // g, u ping-pong, f
+    float *Y_level = nullptr;                 // binned data for a coarse level
+    double *red_partial = nullptr;            // reduction partials
+    double *red_out = nullptr;                // 2 doubles
+    double *h_red = nullptr;                  // pinned host mirror of red_out
+    float *host_stage_vol = nullptr, *host_stage_proj = nullptr, *host_stage_vol2 = nullptr;  // device staging for *_host
+    unsigned long long bytes = 0;
+
+    // multigrid
+    cbct_geometry *coarse = nullptr;
+    int coarsen_flags[4] = {0, 0, 0, 0};
+    bool coarse_tried = false;
+
+    size_t n_vox() const { return (size_t)nx * ny * nz; }
+    size_t n_proj() const { return (size_t)na * nu * nv; }
+};
+
+// ---- error handling -----------------------------------------------------------------------
+void cbct_set_error(const char *fmt, ...);
+#define CBCT_CUDA(call)                                                                         \
+    do {                                                                                        \
+        cudaError_t e_ = (call);                                                                \
+        if (e_ != cudaSuccess) {                                                                \
+            cbct_set_error("%s:%d: %s -> %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
+            return CBCT_ERR_CUDA;                                                               \
+        }                                                                                       \
+    } while (0)
+#define CBCT_TRY(call)                        \
+    do {                                      \
+        cbct_status s_ = (call);              \
+        if (s_ != CBCT_OK) return s_;         \
+    } while (0)
+
+extern unsigned long long g_cbct_launches;
+#define CBCT_LAUNCH_CHECK()                                                      \
+    do {                                                                         \
+        ++g_cbct_launches;                                                       \
+        cudaError_t e_ = cudaGetLastError();                                     \
+        if (e_ != cudaSuccess) {                                                 \
+            cbct_set_error("%s:%d: kernel launch -> %s", __FILE__, __LINE__, cudaGetErrorString(e_)); \
+            return CBCT_ERR_CUDA;                                                \
+        }                                                                        \
+    } while (0)
+
+// ---- per-kernel-class event timing (profile.cu) ---------------------------------------------
+struct ProfileScope {
+    ProfileScope(int tag, cudaStream_t st);
+    ~ProfileScope();
+    int tag_;
+    cudaStream_t st_;
+    cudaEvent_t a_;
+};
+
+// ---- scratch ------------------------------------------------------------------------------
+cbct_status cbct_dev_alloc(cbct_geometry *g, void **p, size_t bytes, bool zero);
+template <typename T>
+inline cbct_status ensure(cbct_geometry *g, T **p, size_t count, bool zero = false)
+{
+    if (*p) return CBCT_OK;
+    return cbct_dev_alloc(g, (void **)p, count * sizeof(T), zero);
+}
+inline size_t pad_elems(const cbct_geometry *g, int c)
+{
+    return (size_t)(g->nz + 2 * kPadK) * (size_t)g->dev.cls[c].plane_stride;
+}
+
+// ---- operators (device pointers, async on stream) ---------------------------------------------
+// projector.cu
+cbct_status op_pad_copies(cbct_geometry *g, const float *d_vol, cudaStream_t st);
+// mode 0: out = P f ; mode 1: out = l * (P f - Y)  (scaled residual for the gather)
+cbct_status op_forward_padded(cbct_geometry *g, float *d_out, const float *d_Y, int mode, cudaStream_t st);
+cbct_status op_scale_proj(cbct_geometry *g, const float *d_proj, float *d_out, cudaStream_t st);
+// backprojector.cu : gathers of the (already l-scaled) projections into G_cls[0], G_cls[1]
+cbct_status op_backproject_gather(cbct_geometry *g, const float *d_scaled, cudaStream_t st);
+// out = G1 + G0^T                         (f == nullptr)
+// out = f - c (G1 + G0^T), optionally clamped at 0   (f != nullptr)
+cbct_status op_combine(cbct_geometry *g, const float *f, float c, int clamp, float *out, cudaStream_t st);
+// tv.cu
+cbct_status op_tv_sweep(cbct_geometry *g, const float *u_in, const float *gv, float *u_out,
+                        float beta, float eps, float dt, int clamp, cudaStream_t st);
+cbct_status op_tv_value(cbct_geometry *g, const float *f, float eps, double *d_out, cudaStream_t st);
+// transfers.cu
+cbct_status op_prolong(cbct_geometry *fine, const float *c, float *f, cudaStream_t st);
+cbct_status op_restrict(cbct_geometry *fine, const float *f, float *c, cudaStream_t st);
+cbct_status op_bin2x2(cbct_geometry *fine, const float *y, float *yc, cudaStream_t st);
+cbct_status op_sumsq_diff(cbct_geometry *g, const float *a, const float *b, size_t n, double *d_out, cudaStream_t st);
+cbct_status op_clamp_copy(cbct_geometry *g, const float *in, float *out, size_t n, cudaStream_t st);

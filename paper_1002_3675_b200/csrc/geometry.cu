@@ -1,0 +1,283 @@
+// Geometry handle: validation, fp64 ray tables, coarse levels, scratch bookkeeping.
+// Convention O0 of DESIGN.md (the paper fixes none of it).
+#include <cmath>
+#include <cstdarg>
+#include <cstring>
+#include <new>
+
+#include "cbct_internal.h"
+
+unsigned long long g_cbct_launches = 0;
+static thread_local char t_err[512] = "";
+
+void cbct_set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(t_err, sizeof(t_err), fmt, ap);
+    va_end(ap);
+}
+
+extern "C" const char *cbct_last_error(void) { return t_err; }
+extern "C" unsigned long long cbct_launch_count(void) { return g_cbct_launches; }
+
+cbct_status cbct_dev_alloc(cbct_geometry *g, void **p, size_t bytes, bool zero)
+{
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) {
+        *p = nullptr;
+        cudaGetLastError();
+        cbct_set_error("cudaMalloc(%zu bytes) failed: %s", bytes, cudaGetErrorString(e));
+        return CBCT_ERR_ALLOC;
+    }
+    if (zero) CBCT_CUDA(cudaMemset(*p, 0, bytes));
+    g->bytes += bytes;
+    return CBCT_OK;
+}
+
+static void free_handle(cbct_geometry *g)
+{
+    if (!g) return;
+    free_handle(g->coarse);
+    void *ptrs[] = {g->d_rays, g->d_zeta, g->d_inv_zeta, g->d_dz, g->d_cs, g->d_tiles[0], g->d_tiles[1],
+                    g->d_angle_has[0], g->d_angle_has[1], g->vol_pad[0], g->vol_pad[1], g->proj_tmp,
+                    g->G_cls[0], g->G_cls[1], g->vol_a, g->vol_b, g->vol_c, g->vol_f, g->Y_level,
+                    g->red_partial, g->red_out, g->host_stage_vol, g->host_stage_proj, g->host_stage_vol2};
+    for (void *p : ptrs)
+        if (p) cudaFree(p);
+    if (g->h_red) cudaFreeHost(g->h_red);
+    delete g;
+}
+
+extern "C" void cbct_geometry_destroy(cbct_geometry *g)
+{
+    if (!g) return;
+    cudaDeviceSynchronize();
+    free_handle(g);
+}
+
+extern "C" unsigned long long cbct_device_bytes(const cbct_geometry *g)
+{
+    unsigned long long b = 0;
+    for (const cbct_geometry *q = g; q; q = q->coarse) b += q->bytes;
+    return b;
+}
+
+extern "C" cbct_status cbct_geometry_query(const cbct_geometry *g, int *d6, double *s5)
+{
+    if (!g) { cbct_set_error("cbct_geometry_query: NULL handle"); return CBCT_ERR_INVALID_ARG; }
+    if (d6) { d6[0] = g->na; d6[1] = g->nu; d6[2] = g->nv; d6[3] = g->nx; d6[4] = g->ny; d6[5] = g->nz; }
+    if (s5) { s5[0] = g->du; s5[1] = g->dv; s5[2] = g->hx; s5[3] = g->hy; s5[4] = g->hz; }
+    return CBCT_OK;
+}
+
+template <typename T>
+static cbct_status upload(cbct_geometry *g, T **dst, const std::vector<T> &src)
+{
+    if (src.empty()) { *dst = nullptr; return CBCT_OK; }
+    CBCT_TRY(cbct_dev_alloc(g, (void **)dst, src.size() * sizeof(T), false));
+    CBCT_CUDA(cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return CBCT_OK;
+}
+
+static cbct_status build_tables(cbct_geometry *g)
+{
+    const int na = g->na, nu = g->nu, nv = g->nv;
+    DevGeom &d = g->dev;
+    d.na = na; d.nu = nu; d.nv = nv; d.nx = g->nx; d.ny = g->ny; d.nz = g->nz;
+    d.koff = g->nz / 2;
+    d.zfrac = (float)(0.5 * g->nz - d.koff);
+    d.hx = (float)g->hx; d.hy = (float)g->hy; d.hz = (float)g->hz;
+    d.du = (float)g->du; d.dv = (float)g->dv; d.sad = (float)g->sad; d.sdd = (float)g->sdd;
+    for (int c = 0; c < 2; ++c) {
+        ClassGrid &cg = d.cls[c];
+        cg.nmaj = c == 0 ? g->nx : g->ny;
+        cg.nmin = c == 0 ? g->ny : g->nx;
+        cg.hmaj = (float)(c == 0 ? g->hx : g->hy);
+        cg.hmin = (float)(c == 0 ? g->hy : g->hx);
+        cg.ioff = cg.nmaj / 2;
+        cg.joff = cg.nmin / 2;
+        cg.row_stride = ((cg.nmin + kPadLo + kPadHi + 3) / 4) * 4;
+        cg.plane_stride = (long long)cg.nmaj * cg.row_stride;
+    }
+
+    std::vector<RayXY> rays((size_t)na * nu);
+    std::vector<float2> cs(na);
+    std::vector<float> zeta(nv), inv_zeta(nv), dz(nv);
+    double max_abs_zeta = 0.0;
+    for (int v = 0; v < nv; ++v) {
+        double Dz = (v - 0.5 * (nv - 1)) * g->dv;
+        dz[v] = (float)Dz;
+        // A ray with Dz == 0 (centre row of an odd nv) never leaves its z row.  It is given an
+        // infinitesimal positive slope so that sign(sz) and sign(1/sz) agree in the kernels and a
+        // ray lying exactly in a z plane is assigned to the row above it, as floor() would.
+        zeta[v] = Dz != 0.0 ? (float)(Dz / g->hz) : 1e-30f;
+        inv_zeta[v] = Dz != 0.0 ? (float)(g->hz / Dz) : 1e30f;
+        max_abs_zeta = std::fmax(max_abs_zeta, std::fabs(Dz / g->hz));
+    }
+    std::vector<int2> tiles[2];
+    double max_abs_dt = 0.0;
+    for (int c = 0; c < 2; ++c) g->h_angle_has[c].assign(na, 0);
+    for (int a = 0; a < na; ++a) {
+        const double th = g->angles[a], co = std::cos(th), si = std::sin(th);
+        cs[a] = make_float2((float)co, (float)si);
+        const double Sx = g->sad * co, Sy = g->sad * si;
+        for (int u = 0; u < nu; ++u) {
+            const double uc = (u - 0.5 * (nu - 1)) * g->du;
+            const double Dx = -(g->sdd - g->sad) * co - uc * si;
+            const double Dy = -(g->sdd - g->sad) * si + uc * co;
+            const double dXv = (Dx - Sx) / g->hx, dYv = (Dy - Sy) / g->hy;
+            const int c = std::fabs(dXv) >= std::fabs(dYv) ? 0 : 1;
+            const ClassGrid &cg = d.cls[c];
+            const double Smaj = c == 0 ? Sx : Sy, Smin = c == 0 ? Sy : Sx;
+            const double dmaj = c == 0 ? Dx - Sx : Dy - Sy, dmin = c == 0 ? Dy - Sy : Dx - Sx;
+            const double hmaj = c == 0 ? g->hx : g->hy;
+            const double hmin = c == 0 ? g->hy : g->hx;
+            const double sm = (dmin / hmin) / (dmaj / hmaj);
+            const double dt = hmaj / dmaj;
+            const double tc = ((cg.ioff - 0.5 * cg.nmaj) * hmaj - Smaj) / dmaj;
+            const double mcu = (Smin + tc * dmin) / hmin + 0.5 * cg.nmin;   // un-centred minor coordinate at plane ioff
+            RayXY r;
+            r.mc = (float)(mcu - cg.joff);
+            r.sm = (float)sm;
+            r.inv_sm = sm != 0.0 ? (float)(1.0 / sm) : 1e30f;
+            if ((float)sm == 0.f) r.inv_sm = 1e30f;
+            r.tc = (float)tc;
+            r.dt = (float)dt;
+            r.inv_dt = (float)(1.0 / dt);
+            r.lxy2 = (float)(hmaj * hmaj + sm * hmin * sm * hmin);
+            // slabs i (between major planes i and i+1) where the minor coordinate can lie in [-1, nmin+1]
+            int ilo = 0, ihi = cg.nmaj;
+            if (sm != 0.0) {
+                double e0 = (-1.0 - mcu) / sm, e1 = (cg.nmin + 1.0 - mcu) / sm;
+                double lo = std::fmin(e0, e1) + cg.ioff, hi = std::fmax(e0, e1) + cg.ioff;
+                double flo = std::floor(lo) - 1.0, fhi = std::ceil(hi) + 1.0;
+                if (flo > ilo) ilo = flo > cg.nmaj ? cg.nmaj : (int)flo;
+                if (fhi < ihi) ihi = fhi < 0 ? 0 : (int)fhi;
+            } else if (mcu < -1.0 || mcu > cg.nmin + 1.0) {
+                ihi = 0;
+            }
+            if (ihi < ilo) ihi = ilo;
+            r.range = ilo | (ihi << 15) | (c << 30);
+            rays[(size_t)a * nu + u] = r;
+            if (ihi > ilo) {
+                g->h_angle_has[c][a] = 1;
+                max_abs_dt = std::fmax(max_abs_dt, std::fabs(dt));
+            }
+        }
+        for (int c = 0; c < 2; ++c)
+            for (int u0 = 0; u0 < nu; u0 += 32) {
+                bool any = false;
+                for (int u = u0; u < u0 + 32 && u < nu; ++u) {
+                    const RayXY &r = rays[(size_t)a * nu + u];
+                    if (ray_cls(r.range) == c && ray_ihi(r.range) > ray_ilo(r.range)) any = true;
+                }
+                if (any) tiles[c].push_back(make_int2(a, u0));
+            }
+    }
+    g->max_abs_sz = (float)(max_abs_dt * max_abs_zeta);
+    if (g->max_abs_sz > 0.999f) {
+        cbct_set_error("geometry unsupported: a ray climbs %.3f voxels in z per major-axis voxel (limit 0.999)",
+                       g->max_abs_sz);
+        return CBCT_ERR_SHAPE;
+    }
+    CBCT_TRY(upload(g, &g->d_rays, rays));
+    CBCT_TRY(upload(g, &g->d_cs, cs));
+    CBCT_TRY(upload(g, &g->d_zeta, zeta));
+    CBCT_TRY(upload(g, &g->d_inv_zeta, inv_zeta));
+    CBCT_TRY(upload(g, &g->d_dz, dz));
+    for (int c = 0; c < 2; ++c) {
+        g->n_tiles[c] = (int)tiles[c].size();
+        CBCT_TRY(upload(g, &g->d_tiles[c], tiles[c]));
+        CBCT_TRY(upload(g, &g->d_angle_has[c], g->h_angle_has[c]));
+    }
+    d.rays = g->d_rays; d.cs = g->d_cs; d.zeta = g->d_zeta; d.inv_zeta = g->d_inv_zeta; d.dz_mm = g->d_dz;
+    return CBCT_OK;
+}
+
+static cbct_status create_impl(double sad, double sdd, const double *angles, int na, int nu, int nv,
+                               double du, double dv, int nx, int ny, int nz, double hx, double hy, double hz,
+                               cbct_geometry **out)
+{
+    if (!out) { cbct_set_error("cbct_geometry_create: out is NULL"); return CBCT_ERR_INVALID_ARG; }
+    *out = nullptr;
+    if (!angles || na <= 0 || nu <= 0 || nv <= 0 || nx <= 0 || ny <= 0 || nz <= 0 ||
+        !(du > 0) || !(dv > 0) || !(hx > 0) || !(hy > 0) || !(hz > 0) || !(sad > 0) || !(sdd > sad)) {
+        cbct_set_error("cbct_geometry_create: NULL angles, non-positive size, or sad >= sdd");
+        return CBCT_ERR_INVALID_ARG;
+    }
+    for (int a = 0; a < na; ++a)
+        if (!std::isfinite(angles[a])) { cbct_set_error("cbct_geometry_create: non-finite angle"); return CBCT_ERR_INVALID_ARG; }
+    if (nx > 16384 || ny > 16384 || nz > 16384 || nu > 16384 || nv > 16384) {
+        cbct_set_error("cbct_geometry_create: a dimension exceeds 16384");
+        return CBCT_ERR_SHAPE;
+    }
+    const double rad = 0.5 * std::hypot(nx * hx, ny * hy);
+    if (!(rad < sad) || !(rad < sdd - sad)) {
+        cbct_set_error("cbct_geometry_create: the volume's circumscribed cylinder (r=%.1f mm) is not strictly "
+                       "between source (%.1f) and detector (%.1f)", rad, sad, sdd - sad);
+        return CBCT_ERR_SHAPE;
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        cbct_set_error("no CUDA device (libcbct has no CPU fallback)");
+        return CBCT_ERR_CUDA;
+    }
+    cbct_geometry *g = new (std::nothrow) cbct_geometry();
+    if (!g) { cbct_set_error("out of host memory"); return CBCT_ERR_ALLOC; }
+    g->sad = sad; g->sdd = sdd; g->du = du; g->dv = dv; g->hx = hx; g->hy = hy; g->hz = hz;
+    g->na = na; g->nu = nu; g->nv = nv; g->nx = nx; g->ny = ny; g->nz = nz;
+    g->angles.assign(angles, angles + na);
+    cbct_status s = build_tables(g);
+    if (s != CBCT_OK) { free_handle(g); return s; }
+    *out = g;
+    return CBCT_OK;
+}
+
+extern "C" cbct_status cbct_geometry_create(double sad, double sdd, const double *angles, int na, int nu, int nv,
+                                            double du, double dv, int nx, int ny, int nz,
+                                            double hx, double hy, double hz, cbct_geometry **out)
+{
+    return create_impl(sad, sdd, angles, na, nu, nv, du, dv, nx, ny, nz, hx, hy, hz, out);
+}
+
+// O6 coarsening rule (Q11): axes with spacing <= sqrt(2) * min spacing halve; detector bins iff x and y did.
+extern "C" cbct_status cbct_geometry_coarsen(const cbct_geometry *gc, cbct_geometry **out, int *flags4)
+{
+    cbct_geometry *g = const_cast<cbct_geometry *>(gc);
+    if (!g || !out) { cbct_set_error("cbct_geometry_coarsen: NULL argument"); return CBCT_ERR_INVALID_ARG; }
+    if (!g->coarse) {
+        const double h[3] = {g->hx, g->hy, g->hz};
+        int n[3] = {g->nx, g->ny, g->nz};
+        double hn[3] = {g->hx, g->hy, g->hz};
+        const double m = std::fmin(h[0], std::fmin(h[1], h[2]));
+        int fl[4] = {0, 0, 0, 0};
+        for (int a = 0; a < 3; ++a) {
+            if (h[a] <= std::sqrt(2.0) * m * (1.0 + 1e-9)) {
+                if (n[a] % 2) {
+                    cbct_set_error("cbct_geometry_coarsen: odd dimension %d on an axis that must coarsen", n[a]);
+                    return CBCT_ERR_SHAPE;
+                }
+                fl[a] = 1; n[a] /= 2; hn[a] *= 2.0;
+            }
+        }
+        int nu = g->nu, nv = g->nv;
+        double du = g->du, dv = g->dv;
+        if (fl[0] && fl[1]) {
+            if (nu % 2 || nv % 2) {
+                cbct_set_error("cbct_geometry_coarsen: odd detector dimension on a level that bins the detector");
+                return CBCT_ERR_SHAPE;
+            }
+            fl[3] = 1; nu /= 2; nv /= 2; du *= 2.0; dv *= 2.0;
+        }
+        cbct_geometry *c = nullptr;
+        CBCT_TRY(create_impl(g->sad, g->sdd, g->angles.data(), g->na, nu, nv, du, dv, n[0], n[1], n[2],
+                             hn[0], hn[1], hn[2], &c));
+        g->coarse = c;
+        std::memcpy(g->coarsen_flags, fl, sizeof(fl));
+    }
+    *out = g->coarse;
+    if (flags4) std::memcpy(flags4, g->coarsen_flags, sizeof(g->coarsen_flags));
+    return CBCT_OK;
+}

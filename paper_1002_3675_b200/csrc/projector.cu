@@ -1,0 +1,206 @@
+// a1/a2: ray-driven exact-chord cone-beam projector (definition O1 in DESIGN.md).
+//
+// One thread marches V rays that share a detector column u (and therefore share their whole
+// x-y traversal: the detector's v axis is parallel to the rotation axis, so the t-parameters of
+// all x- and y-plane crossings are independent of v).  A warp is 32 adjacent u of one
+// detector-row group, so in every slab its lanes read ~contiguous minor-axis addresses of the
+// class' padded volume copy (class 0 reads the [k][x][y] transposed copy, class 1 the [k][y][x]
+// copy).  Per slab (one voxel of the major axis) a ray touches at most two minor rows, split at
+// lambda = a, and at most two z rows, split at lambda = b (lambda = position inside the slab
+// in [0,1]); the four chord fractions are
+//      (r0,k0) min(a,b)   (r1,k0) b - min(a,b)   (r0,k1) a - min(a,b)   (r1,k1) 1 - max(a,b)
+// and the backprojector (backprojector.cu) evaluates exactly the same expressions.
+#include "cbct_internal.h"
+#include "ray_common.cuh"
+
+// ------------------------------------------------------------------------------------------
+// Padded copies: class 1 copy is [k+K][j][PadLo+i], class 0 copy is the transpose [k+K][i][PadLo+j].
+// Pads are zeroed once at allocation and never written, which is what makes "f = 0 outside
+// the volume" exact without bounds checks in the march.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) pad_copy_kernel(const float *__restrict__ vol, float *__restrict__ pad_x,
+                                                       float *__restrict__ pad_y, int nx, int ny,
+                                                       int rs_x, long long ps_x, int rs_y, long long ps_y)
+{
+    __shared__ float tile[32][33];
+    const int k = blockIdx.z;
+    const int i0 = blockIdx.x * 32, j0 = blockIdx.y * 32;
+    const float *src = vol + (size_t)k * ny * nx;
+    for (int r = threadIdx.y; r < 32; r += 8) {
+        int j = j0 + r, i = i0 + threadIdx.x;
+        float v = (j < ny && i < nx) ? __ldg(src + (size_t)j * nx + i) : 0.f;
+        tile[r][threadIdx.x] = v;
+        if (pad_y && j < ny && i < nx) pad_y[(size_t)(k + kPadK) * ps_y + (size_t)j * rs_y + kPadLo + i] = v;
+    }
+    if (!pad_x) return;
+    __syncthreads();
+    for (int r = threadIdx.y; r < 32; r += 8) {
+        int i = i0 + r, j = j0 + threadIdx.x;
+        if (i < nx && j < ny) pad_x[(size_t)(k + kPadK) * ps_x + (size_t)i * rs_x + kPadLo + j] = tile[threadIdx.x][r];
+    }
+}
+
+cbct_status op_pad_copies(cbct_geometry *g, const float *d_vol, cudaStream_t st)
+{
+    for (int c = 0; c < 2; ++c)
+        if (g->n_tiles[c] > 0) CBCT_TRY(ensure(g, &g->vol_pad[c], pad_elems(g, c), true));
+    float *px = g->n_tiles[0] > 0 ? g->vol_pad[0] : nullptr;
+    float *py = g->n_tiles[1] > 0 ? g->vol_pad[1] : nullptr;
+    if (!px && !py) return CBCT_OK;
+    const DevGeom &d = g->dev;
+    ProfileScope ps(0, st);
+    dim3 grid((g->nx + 31) / 32, (g->ny + 31) / 32, g->nz), block(32, 8);
+    pad_copy_kernel<<<grid, block, 0, st>>>(d_vol, px, py, g->nx, g->ny, d.cls[0].row_stride, d.cls[0].plane_stride,
+                                            d.cls[1].row_stride, d.cls[1].plane_stride);
+    CBCT_LAUNCH_CHECK();
+    return CBCT_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// Forward march.
+// ------------------------------------------------------------------------------------------
+template <int V, int WARPS>
+__global__ void __launch_bounds__(32 * WARPS)
+forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, const float *__restrict__ vol,
+               float *__restrict__ out, const float *__restrict__ Y, const int mode)
+{
+    const ClassGrid cg = d.cls[cls];
+    const int lane = threadIdx.x;
+    const int2 tile = tiles[blockIdx.x];
+    const int a = tile.x, u = tile.y + lane;
+    const int v0 = (blockIdx.y * WARPS + threadIdx.y) * V;
+    if (v0 >= d.nv) return;                                   // warp-uniform
+
+    RayXY r = load_ray(d, a, min(u, d.nu - 1));
+    int ilo = ray_ilo(r.range), ihi = ray_ihi(r.range);
+    const bool mine = (u < d.nu) && (ray_cls(r.range) == cls);
+    bool active = mine && ihi > ilo;
+
+    // z clip: the ray of this thread closest to the central plane stays inside longest
+    {
+        const float za = __ldg(d.zeta + v0), zb = __ldg(d.zeta + min(v0 + V - 1, d.nv - 1));
+        float tmax = 3.0e38f;
+        if (za > 0.f && zb > 0.f) tmax = ((float)(d.nz - d.koff) + 1.f - d.zfrac) / fminf(za, zb);
+        else if (za < 0.f && zb < 0.f) tmax = (-(float)d.koff - 1.f - d.zfrac) / fmaxf(za, zb);
+        if (tmax < 2.f) {                                     // t <= tmax, t = tc + (i - ioff) dt
+            float e = (tmax - r.tc) * r.inv_dt;
+            if (r.dt > 0.f) ihi = min(ihi, cg.ioff + (int)floorf(e) + 2);
+            else            ilo = max(ilo, cg.ioff + (int)ceilf(e) - 2);
+        }
+        active = active && ihi > ilo;
+    }
+    if (!active) { r.mc = -30000.f; r.sm = 0.f; r.inv_sm = 1e30f; }   // clamps to the zero pad
+    const int lo_w = __reduce_min_sync(0xffffffffu, active ? ilo : 0x7fffffff);
+    const int hi_w = __reduce_max_sync(0xffffffffu, active ? ihi : -1);
+
+    float acc[V];
+#pragma unroll
+    for (int q = 0; q < V; ++q) acc[q] = 0.f;
+
+    if (lo_w < hi_w) {
+        const float dirpos = r.sm >= 0.f ? 1.f : 0.f;
+        const int dneg = r.sm >= 0.f ? 0 : 1;
+        float zeta[V], inv_sz[V], zbnd[V], zstep[V];
+        long long rowoff[V];
+        const float e0 = (float)(lo_w - cg.ioff);
+        const float T0 = fmaf(e0, r.dt, r.tc);
+#pragma unroll
+        for (int q = 0; q < V; ++q) {
+            const int v = min(v0 + q, d.nv - 1);
+            zeta[q] = __ldg(d.zeta + v);
+            inv_sz[q] = r.inv_dt * __ldg(d.inv_zeta + v);
+            const float sz = r.dt * zeta[q];
+            zstep[q] = sz >= 0.f ? 1.f : -1.f;
+            const float Za = fmaf(T0, zeta[q], d.zfrac);
+            const float kf = floorf(Za);
+            zbnd[q] = kf + (sz >= 0.f ? 1.f : 0.f);
+            const int k = (int)kf + d.koff;
+            rowoff[q] = (long long)(min(max(k, -kPadK), d.nz + kPadK - 1) + kPadK) * cg.plane_stride;
+        }
+        const float *base = vol + kPadLo;
+        for (int i = lo_w; i < hi_w; ++i) {
+            const float ef = (float)(i - cg.ioff);
+            const float T = fmaf(ef, r.dt, r.tc);
+            float a_, fl;
+            minor_split(ef, r, dirpos, a_, fl);
+            const int ja = (int)fl + cg.joff;
+            const int jlo = min(max(ja - dneg, -2), cg.nmin);
+            const float oma = 1.f - a_;
+            const float wlo = dneg ? oma : a_;                 // fraction [0,a] belongs to row ja, [a,1] to ja+dir
+            const float whi = dneg ? a_ : oma;
+            const long long off_i = (long long)i * cg.row_stride + jlo;
+#pragma unroll
+            for (int q = 0; q < V; ++q) {
+                const float Za = fmaf(T, zeta[q], d.zfrac);
+                const float b = __saturatef((zbnd[q] - Za) * inv_sz[q]);
+                const float *p = base + rowoff[q] + off_i;
+                if (!__any_sync(0xffffffffu, b < 1.f)) {
+                    acc[q] = fmaf(wlo, __ldg(p), acc[q]);
+                    acc[q] = fmaf(whi, __ldg(p + 1), acc[q]);
+                } else {
+                    // z-plane crossing inside this slab for some lane: general four-term form
+                    const int k1 = (int)(zbnd[q] - (zstep[q] > 0.f ? 1.f : 0.f) + zstep[q]) + d.koff;
+                    const long long rowoff1 = (long long)(min(max(k1, -kPadK), d.nz + kPadK - 1) + kPadK) * cg.plane_stride;
+                    const float *p1 = base + rowoff1 + off_i;
+                    const float mn = fminf(a_, b), mx = fmaxf(a_, b);
+                    const float w_r0k0 = mn, w_r1k0 = b - mn, w_r0k1 = a_ - mn, w_r1k1 = 1.f - mx;
+                    const float wl0 = dneg ? w_r1k0 : w_r0k0, wh0 = dneg ? w_r0k0 : w_r1k0;
+                    const float wl1 = dneg ? w_r1k1 : w_r0k1, wh1 = dneg ? w_r0k1 : w_r1k1;
+                    float s = wl0 * __ldg(p);
+                    s = fmaf(wh0, __ldg(p + 1), s);
+                    s = fmaf(wl1, __ldg(p1), s);
+                    s = fmaf(wh1, __ldg(p1 + 1), s);
+                    acc[q] += s;
+                    if (b < 1.f) { zbnd[q] += zstep[q]; rowoff[q] = rowoff1; }
+                }
+            }
+        }
+    }
+    if (!mine) return;
+#pragma unroll
+    for (int q = 0; q < V; ++q) {
+        const int v = v0 + q;
+        if (v < d.nv) {
+            const float len = chord_scale(r, __ldg(d.dz_mm + v));
+            const size_t o = ((size_t)a * d.nv + v) * d.nu + u;
+            float val = len * acc[q];
+            if (mode == 1) val = len * (val - __ldg(Y + o));
+            out[o] = val;
+        }
+    }
+}
+
+cbct_status op_forward_padded(cbct_geometry *g, float *d_out, const float *d_Y, int mode, cudaStream_t st)
+{
+    constexpr int V = 8, WARPS = 4;
+    ProfileScope ps(1, st);
+    // rays in no tile miss the volume: P f = 0 there
+    if (mode == 0) CBCT_CUDA(cudaMemsetAsync(d_out, 0, g->n_proj() * sizeof(float), st));
+    for (int c = 0; c < 2; ++c) {
+        if (g->n_tiles[c] == 0) continue;
+        dim3 grid(g->n_tiles[c], (g->nv + V * WARPS - 1) / (V * WARPS)), block(32, WARPS);
+        forward_kernel<V, WARPS><<<grid, block, 0, st>>>(g->dev, c, g->d_tiles[c], g->vol_pad[c], d_out, d_Y, mode);
+        CBCT_LAUNCH_CHECK();
+    }
+    return CBCT_OK;
+}
+
+// scaled copy for the gather: out = l(u,v) * proj
+__global__ void __launch_bounds__(256) scale_proj_kernel(const DevGeom d, const float *__restrict__ in, float *__restrict__ out)
+{
+    const int u = blockIdx.x * blockDim.x + threadIdx.x;
+    const int v = blockIdx.y, a = blockIdx.z;
+    if (u >= d.nu) return;
+    const RayXY r = load_ray(d, a, u);
+    const size_t o = ((size_t)a * d.nv + v) * d.nu + u;
+    out[o] = chord_scale(r, __ldg(d.dz_mm + v)) * __ldg(in + o);
+}
+
+cbct_status op_scale_proj(cbct_geometry *g, const float *d_proj, float *d_out, cudaStream_t st)
+{
+    ProfileScope ps(2, st);
+    dim3 grid((g->nu + 255) / 256, g->nv, g->na);
+    scale_proj_kernel<<<grid, 256, 0, st>>>(g->dev, d_proj, d_out);
+    CBCT_LAUNCH_CHECK();
+    return CBCT_OK;
+}

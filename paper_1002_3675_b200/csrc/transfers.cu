@@ -1,0 +1,118 @@
+// a7: multigrid transfers of the coarse-to-fine cascade ("multi-grid method"; O6/Q11 in DESIGN.md).
+// All HBM-bound pointwise kernels.
+#include "cbct_internal.h"
+
+namespace {
+// fine[2I] = 3/4 c[I] + 1/4 c[I-1], fine[2I+1] = 3/4 c[I] + 1/4 c[I+1] (clamped) on coarsened axes.
+__device__ __forceinline__ void lin_pair(int fine, int ncoarse, bool coarsened, int &i0, int &i1, float &w1)
+{
+    if (!coarsened) { i0 = fine; i1 = fine; w1 = 0.f; return; }
+    i0 = fine >> 1;
+    i1 = (fine & 1) ? min(i0 + 1, ncoarse - 1) : max(i0 - 1, 0);
+    w1 = 0.25f;
+}
+
+__global__ void __launch_bounds__(256)
+prolong_kernel(const float *__restrict__ c, float *__restrict__ f, int nx, int ny, int nz,
+               int cx, int cy, int cz, int ax, int ay, int az)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y, k = blockIdx.z;
+    if (i >= nx) return;
+    int i0, i1, j0, j1, k0, k1;
+    float wi, wj, wk;
+    lin_pair(i, cx, ax, i0, i1, wi);
+    lin_pair(j, cy, ay, j0, j1, wj);
+    lin_pair(k, cz, az, k0, k1, wk);
+    auto at = [&](int kk, int jj, int ii) { return __ldg(c + ((size_t)kk * cy + jj) * cx + ii); };
+    auto lx = [&](int kk, int jj) { return fmaf(wi, at(kk, jj, i1), (1.f - wi) * at(kk, jj, i0)); };
+    auto ly = [&](int kk) { return fmaf(wj, lx(kk, j1), (1.f - wj) * lx(kk, j0)); };
+    f[((size_t)k * ny + j) * nx + i] = fmaf(wk, ly(k1), (1.f - wk) * ly(k0));
+}
+
+__global__ void __launch_bounds__(256)
+restrict_kernel(const float *__restrict__ f, float *__restrict__ c, int nx, int ny, int cx, int cy, int cz,
+                int ax, int ay, int az)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y, k = blockIdx.z;
+    if (i >= cx) return;
+    const int sx = ax ? 2 : 1, sy = ay ? 2 : 1, sz = az ? 2 : 1;
+    float acc = 0.f;
+    for (int dk = 0; dk < sz; ++dk)
+        for (int dj = 0; dj < sy; ++dj)
+            for (int di = 0; di < sx; ++di)
+                acc += __ldg(f + ((size_t)(k * sz + dk) * ny + (j * sy + dj)) * nx + (i * sx + di));
+    c[((size_t)k * cy + j) * cx + i] = acc / (float)(sx * sy * sz);
+}
+
+__global__ void __launch_bounds__(256)
+bin2x2_kernel(const float *__restrict__ y, float *__restrict__ yc, int nu, int nv, int cu, int cv)
+{
+    const int u = blockIdx.x * blockDim.x + threadIdx.x;
+    const int v = blockIdx.y, a = blockIdx.z;
+    if (u >= cu) return;
+    const float *p = y + ((size_t)a * nv + 2 * v) * nu + 2 * u;
+    const float2 r0 = __ldg(reinterpret_cast<const float2 *>(p));
+    const float2 r1 = __ldg(reinterpret_cast<const float2 *>(p + nu));
+    yc[((size_t)a * cv + v) * cu + u] = 0.25f * ((r0.x + r0.y) + (r1.x + r1.y));
+}
+
+__global__ void __launch_bounds__(256) clamp_copy_kernel(const float *__restrict__ in, float *__restrict__ out, size_t n)
+{
+    for (size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x; o < n; o += (size_t)gridDim.x * blockDim.x)
+        out[o] = fmaxf(__ldg(in + o), 0.f);
+}
+}  // namespace
+
+static cbct_status need_coarse(cbct_geometry *fine, cbct_geometry **c)
+{
+    return cbct_geometry_coarsen(fine, c, nullptr);
+}
+
+cbct_status op_prolong(cbct_geometry *fine, const float *c, float *f, cudaStream_t st)
+{
+    cbct_geometry *gc;
+    CBCT_TRY(need_coarse(fine, &gc));
+    const int *fl = fine->coarsen_flags;
+    ProfileScope ps(6, st);
+    dim3 grid((fine->nx + 255) / 256, fine->ny, fine->nz);
+    prolong_kernel<<<grid, 256, 0, st>>>(c, f, fine->nx, fine->ny, fine->nz, gc->nx, gc->ny, gc->nz, fl[0], fl[1], fl[2]);
+    CBCT_LAUNCH_CHECK();
+    return CBCT_OK;
+}
+
+cbct_status op_restrict(cbct_geometry *fine, const float *f, float *c, cudaStream_t st)
+{
+    cbct_geometry *gc;
+    CBCT_TRY(need_coarse(fine, &gc));
+    const int *fl = fine->coarsen_flags;
+    ProfileScope ps(6, st);
+    dim3 grid((gc->nx + 255) / 256, gc->ny, gc->nz);
+    restrict_kernel<<<grid, 256, 0, st>>>(f, c, fine->nx, fine->ny, gc->nx, gc->ny, gc->nz, fl[0], fl[1], fl[2]);
+    CBCT_LAUNCH_CHECK();
+    return CBCT_OK;
+}
+
+cbct_status op_bin2x2(cbct_geometry *fine, const float *y, float *yc, cudaStream_t st)
+{
+    cbct_geometry *gc;
+    CBCT_TRY(need_coarse(fine, &gc));
+    if (!fine->coarsen_flags[3]) {
+        CBCT_CUDA(cudaMemcpyAsync(yc, y, fine->n_proj() * sizeof(float), cudaMemcpyDeviceToDevice, st));
+        return CBCT_OK;
+    }
+    ProfileScope ps(6, st);
+    dim3 grid((gc->nu + 255) / 256, gc->nv, gc->na);
+    bin2x2_kernel<<<grid, 256, 0, st>>>(y, yc, fine->nu, fine->nv, gc->nu, gc->nv);
+    CBCT_LAUNCH_CHECK();
+    return CBCT_OK;
+}
+
+cbct_status op_clamp_copy(cbct_geometry *g, const float *in, float *out, size_t n, cudaStream_t st)
+{
+    (void)g;
+    clamp_copy_kernel<<<1184, 256, 0, st>>>(in, out, n);
+    CBCT_LAUNCH_CHECK();
+    return CBCT_OK;
+}

@@ -1,0 +1,118 @@
+"""Parity at BASELINE.json's full sizes (c2..c5), in the launch configuration bench.py times, on
+sampled outputs the oracle computes one by one (single rays by traversal, single voxels by brute-force
+clipping), plus properties that hold at any size and one full-size loop iteration for c3."""
+import numpy as np
+import pytest
+
+import oracle as o
+from cbct_synth import make_config, gaussian_field
+
+pytestmark = pytest.mark.gpu
+
+
+def f32(a):
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+def rel(a, b):
+    a = np.asarray(a, dtype=np.float64)
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+def sampled_operator_parity(cb, cfg, n_rays=4000, n_vox=600, angle_subset=None, adjoint=True):
+    import torch
+    dev = torch.device("cuda:0")
+    g = cfg.geom if angle_subset is None else cfg.geom.with_angles(cfg.geom.angles[angle_subset])
+    G = cb.Geometry.from_synth(g)
+    vol = f32(cfg.volume())
+    d_vol = torch.from_numpy(vol).to(dev)
+    d_q = torch.empty(g.proj_shape, device=dev)
+    cb.forward(G, d_vol, d_q)
+    rng = np.random.default_rng(cfg.seed + 99)
+    ia, iv, iu = rng.integers(g.n_angles, size=n_rays), rng.integers(g.nv, size=n_rays), rng.integers(g.nu, size=n_rays)
+    # include detector corners / edges and tile boundaries
+    iv[:8] = [0, 0, g.nv - 1, g.nv - 1, g.nv // 2, g.nv // 2 - 1, 31, 32]
+    iu[:8] = [0, g.nu - 1, 0, g.nu - 1, g.nu // 2, g.nu // 2 - 1, 31, 32]
+    q = d_q.cpu().numpy()
+    ref = o.forward_rays(g, vol.astype(np.float64), ia, iv, iu)
+    e_fwd = rel(q[ia, iv, iu], ref)
+    # backproject P(phantom); sampled voxels by brute-force clipping
+    d_b = torch.empty(g.vol_shape, device=dev)
+    cb.backproject(G, d_q, d_b)
+    ix, iy, iz = rng.integers(g.nx, size=n_vox), rng.integers(g.ny, size=n_vox), rng.integers(g.nz, size=n_vox)
+    ix[:6] = [0, g.nx - 1, 0, g.nx // 2, 31, 32]
+    iy[:6] = [0, g.ny - 1, g.ny - 1, g.ny // 2, 32, 31]
+    iz[:6] = [0, g.nz - 1, g.nz // 2, 0, 15, 16]
+    b = d_b.cpu().numpy()
+    bref = o.backproject_voxels(g, q.astype(np.float64), ix, iy, iz)
+    e_bp = rel(b[iz, iy, ix], bref)
+    e_adj = None
+    if adjoint:
+        x = torch.from_numpy(f32(gaussian_field(g.vol_shape, 11))).to(dev)
+        y = torch.from_numpy(f32(gaussian_field(g.proj_shape, 12))).to(dev)
+        Px = torch.empty(g.proj_shape, device=dev)
+        Pty = torch.empty(g.vol_shape, device=dev)
+        cb.forward(G, x, Px)
+        cb.backproject(G, y, Pty)
+        lhs = float((Px.double() * y.double()).sum())
+        rhs = float((x.double() * Pty.double()).sum())
+        e_adj = abs(lhs - rhs) / (float(Px.double().norm()) * float(y.double().norm()))
+    G.close()
+    return e_fwd, e_bp, e_adj
+
+
+def test_c2_operator_bench_config(cuda_lib):
+    """configs[1]: 256^3 volume, 40 views of 512x384 — the workload bench.py times."""
+    e_fwd, e_bp, e_adj = sampled_operator_parity(cuda_lib, make_config("c2"))
+    assert e_fwd <= 1e-5 and e_bp <= 1e-5 and e_adj <= 1e-5, (e_fwd, e_bp, e_adj)
+
+
+@pytest.mark.parametrize("name", ["c3", "c4"])
+def test_c3_c4_operators_full_size(cuda_lib, name):
+    e_fwd, e_bp, e_adj = sampled_operator_parity(cuda_lib, make_config(name))
+    assert e_fwd <= 1e-5 and e_bp <= 1e-5 and e_adj <= 1e-5, (e_fwd, e_bp, e_adj)
+
+
+def test_c3_one_full_size_outer_iteration(cuda_lib):
+    """One outer FBS iteration at the full c3 size (finest level, warm start) against the oracle."""
+    import torch
+    cb = cuda_lib
+    dev = torch.device("cuda:0")
+    cfg = make_config("c3")
+    g = cfg.geom
+    G = cb.Geometry.from_synth(g)
+    Y = f32(cfg.projections())
+    f0 = f32(0.7 * cfg.volume())
+    f = torch.empty(g.vol_shape, device=dev)
+    cb.fbs_reconstruct(G, torch.from_numpy(Y).to(dev), torch.from_numpy(f0).to(dev), 1, [1], cfg.n_inner,
+                       cfg.step, cfg.mu, cfg.eps, cfg.omega, f)
+    ref = o.fbs_reconstruct(g, Y.astype(np.float64), f0.astype(np.float64), 1, [1], cfg.n_inner, cfg.step, cfg.mu,
+                            cfg.eps, cfg.omega)
+    out = f.cpu().numpy()
+    assert rel(out, ref) <= 1e-4
+    # the update itself (not just f0 carried over) matches
+    assert rel(out - f0, ref - f0.astype(np.float64)) <= 2e-4
+    assert out.min() >= 0.0
+    G.close()
+
+
+def test_c5_stress_subsets(cuda_lib):
+    """c5 (512^3, 360 views of 1024x768): operator parity on a fixed 8-angle subset (row blocks of P and
+    partial sums of P^T are exact sub-problems), TV parity on the full volume."""
+    import torch
+    cb = cuda_lib
+    dev = torch.device("cuda:0")
+    cfg = make_config("c5")
+    subset = np.arange(0, 360, 45) + 3
+    e_fwd, e_bp, e_adj = sampled_operator_parity(cb, cfg, n_rays=3000, n_vox=400, angle_subset=subset)
+    assert e_fwd <= 1e-5 and e_bp <= 1e-5 and e_adj <= 1e-5, (e_fwd, e_bp, e_adj)
+    g = cfg.geom.with_angles(cfg.geom.angles[:1])
+    G = cb.Geometry.from_synth(g)
+    rng = np.random.default_rng(77)
+    gv = f32(cfg.volume() + 0.002 * rng.standard_normal(g.vol_shape, dtype=np.float32))
+    d_g = torch.from_numpy(gv).to(dev)
+    u = d_g.clone()
+    cb.tv_prox(G, d_g, u, cfg.beta, cfg.eps, 1.0, 2)
+    ref = o.tv_prox(g, gv.astype(np.float64), gv.astype(np.float64), cfg.beta, cfg.eps, 1.0, 2)
+    assert rel(u.cpu().numpy(), ref) <= 1e-5
+    G.close()
