@@ -227,9 +227,9 @@ def energy(g: Geometry, d_f, d_Y, mu, eps, stream=None):
 
 def _outer(n_levels: int, n_outer: Sequence[int]):
     n_outer = [int(x) for x in n_outer]
-    if len(n_outer) != n_levels:
+    if n_levels >= 1 and len(n_outer) != n_levels:
         raise ValueError("n_outer must list one count per level, coarsest first")
-    return (C.c_int * n_levels)(*n_outer), sum(n_outer)
+    return (C.c_int * max(len(n_outer), 1))(*n_outer), sum(n_outer)    # n_levels < 1 is rejected by the library
 
 
 def fbs_reconstruct(g: Geometry, d_Y, d_f0, n_levels, n_outer, n_inner, step, mu, eps, omega, d_f_out,
