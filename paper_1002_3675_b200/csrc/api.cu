@@ -31,7 +31,7 @@ extern "C" cbct_status cbct_backproject(const cbct_geometry *gc, const float *d_
     cbct_geometry *g = mut(gc);
     cudaStream_t st = (cudaStream_t)stream;
     CBCT_TRY(ensure(g, &g->proj_tmp, g->n_proj(), true));
-    CBCT_TRY(op_scale_proj(g, d_proj, g->proj_tmp, st));
+    CBCT_TRY(op_backproject_prefix(g, d_proj, 1, g->proj_tmp, st));       // l * y and its prefix sums along v
     CBCT_TRY(op_backproject_gather(g, g->proj_tmp, st));
     return op_combine(g, nullptr, 0.f, 0, d_vol, st);
 }
@@ -132,6 +132,7 @@ static cbct_status fbs_level(cbct_geometry *g, const float *d_Y, float *f, int n
     for (int it = 0; it < n_outer; ++it) {
         CBCT_TRY(op_pad_copies(g, f, st));
         CBCT_TRY(op_forward_padded(g, g->proj_tmp, d_Y, 1, st));          // l (P f - Y)          a1+a2
+        CBCT_TRY(op_backproject_prefix(g, g->proj_tmp, 0, nullptr, st));
         CBCT_TRY(op_backproject_gather(g, g->proj_tmp, st));              // P^T (P f - Y)        a3
         if (n_inner == 0) {
             CBCT_TRY(op_combine(g, f, c, 1, g->vol_a, st));               // max(f - c G, 0)      a4+a6

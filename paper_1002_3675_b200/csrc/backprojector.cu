@@ -7,20 +7,66 @@
 //   * in-plane: the rays u whose slab-i traversal touches minor row j.  Candidates come from
 //     projecting the column's x-y square onto the detector; each is then tested with the
 //     projector's own minor_split(), giving its lambda-interval [l0,l1] inside row j;
-//   * axially: for row k the rays v whose z-interval meets [l0,l1]; with p0,p1 the (saturated)
-//     lambdas at which ray v meets planes k and k+1, the chord fraction is
-//         w = max(0, min(l1, max(p0,p1)) - max(l0, min(p0,p1)))
-//     which reproduces the projector's four fractions term by term (see ray_common.cuh).
+//   * axially: within the slab a ray (u,v) lies in at most two z rows, split at lambda = b(u,v).
+//     The rays of column u that ENTER the slab in row k are a contiguous run of v, bounded by the
+//     first ray at or above plane k and the first at or above plane k+1, so
+//         sum_v [entry row = k] y(u,v) = C(u, vT(k+1)) - C(u, vT(k))
+//     with C the prefix sums of y along v (built once per call by prefix_kernel, compensated so
+//     that the difference carries fp32 accuracy).  That is the whole weight (l1 - l0) of every ray
+//     that does not cross a z plane inside the slab (most of them).  A ray that does cross plane k
+//     (its v lies between vT(k) and the same bound taken at the slab's exit plane) moves
+//         max(0, l1 - max(l0, b))        (= its exit-row fraction among the projector's four)
+//     from its entry z row to its exit z row, with b from the projector's own expression.
+//     The cost per (column, ray u) is therefore O(KC), independent of how many detector rows fall
+//     into one voxel row (4.8 at c3's 2.5 mm slices).
 // The projections handed in are pre-multiplied by the slab chord length l(u,v).
 // One launch per ray class; class 0 accumulates into a [k][x][y] array, class 1 into [k][y][x],
 // so lanes (adjacent minor index) write contiguously; op_combine() adds the two.
 #include "cbct_internal.h"
 #include "ray_common.cuh"
 
+// C[a][v][u] = sum_{v' < v} y[a][v'][u] for v = 0..nv as (sum, compensation) pairs: the rounding
+// error of every addition is carried in the second float (two-sum), so C(v2) - C(v1) evaluated as
+// (s2 - s1) + (c2 - c1) has the accuracy of summing the run directly.
+// scale != 0: y = l(u,v) * in (and the scaled projections are also written to rs_out).
+__global__ void __launch_bounds__(128) prefix_kernel(const DevGeom d, const float *__restrict__ in, const int scale,
+                                                     float *__restrict__ rs_out, float2 *__restrict__ C)
+{
+    const int u = blockIdx.x * blockDim.x + threadIdx.x, a = blockIdx.y;
+    if (u >= d.nu) return;
+    RayXY r = load_ray(d, a, u);
+    const float *p = in + (size_t)a * d.nv * d.nu + u;
+    float *po = rs_out ? rs_out + (size_t)a * d.nv * d.nu + u : nullptr;
+    float2 *c = C + (size_t)a * (d.nv + 1) * d.nu + u;
+    float s = 0.f, e = 0.f;
+    *c = make_float2(0.f, 0.f);
+    constexpr int PF = 8;
+    for (int v0 = 0; v0 < d.nv; v0 += PF) {
+        float y[PF];
+#pragma unroll
+        for (int q = 0; q < PF; ++q) y[q] = (v0 + q < d.nv) ? __ldg(p + (size_t)(v0 + q) * d.nu) : 0.f;
+#pragma unroll
+        for (int q = 0; q < PF; ++q) {
+            if (v0 + q >= d.nv) break;
+            float yy = y[q];
+            if (scale) {
+                yy *= chord_scale(r, __ldg(d.dz_mm + v0 + q));
+                if (po) po[(size_t)(v0 + q) * d.nu] = yy;
+            }
+            const float t = s + yy;
+            const float bp = t - s;
+            e += (s - (t - bp)) + (yy - bp);
+            s = t;
+            c[(size_t)(v0 + q + 1) * d.nu] = make_float2(s, e);
+        }
+    }
+}
+
+
 template <int KC, int BI>
 __global__ void __launch_bounds__(32 * BI)
 backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restrict__ angle_has,
-                   const float *__restrict__ rs, float *__restrict__ G)
+                   const float *__restrict__ rs, const float2 *__restrict__ C, float *__restrict__ G)
 {
     const ClassGrid cg = d.cls[cls];
     const int j = blockIdx.x * 32 + threadIdx.x;      // minor index
@@ -41,7 +87,9 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
     const float ef = (float)(i - cg.ioff);
     const float cu = 0.5f * (float)(d.nu - 1), cv = 0.5f * (float)(d.nv - 1);
     const float sdd_du = d.sdd / d.du;
-    const float dzeta = d.dv / d.hz;
+    const float hz_dv = d.hz / d.dv;
+    const float zk0 = (float)(k0 - d.koff) - d.zfrac;  // plane k0 in the units of z_entry(), minus zfrac
+    const size_t cplane = (size_t)(d.nv + 1) * d.nu;
 
     for (int a = 0; a < d.na; ++a) {
         if (!angle_has[a]) continue;                   // uniform
@@ -60,40 +108,50 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
         const int uB = valid ? min(d.nu - 1, (int)ceilf(umax + 0.02f)) : -1;
         for (int u = uA; u <= uB; ++u) {
             const RayXY r = load_ray(d, a, u);
-            if (ray_cls(r.range) != cls || i < ray_ilo(r.range) || i >= ray_ihi(r.range)) continue;
-            const float dirpos = r.sm >= 0.f ? 1.f : 0.f;
+            if (ray_cls(r.range) != cls) continue;
             float a_, fl;
-            minor_split(ef, r, dirpos, a_, fl);
+            minor_split(ef, r, r.sm >= 0.f ? 1.f : 0.f, a_, fl);
             const int ja = (int)fl + cg.joff;
             float l0, l1;
             if (ja == j) { l0 = 0.f; l1 = a_; }
             else if (ja + (r.sm >= 0.f ? 1 : -1) == j) { l0 = a_; l1 = 1.f; }
             else continue;
-            if (!(l1 > l0)) continue;
+            const float w = l1 - l0;
+            if (!(w > 0.f)) continue;
 
-            const float T = fmaf(ef, r.dt, r.tc);
-            const float invB = __fdividef(1.f, T * dzeta);            // d v / d Z at this slab
-            const float absdt_T = fabsf(r.dt) / T;
-            const float *rsa = rs + (size_t)a * d.nv * d.nu + u;
+            const float T = fmaf(ef, r.dt, r.tc), Tn = fmaf(ef + 1.f, r.dt, r.tc);   // entry / exit ray parameter
+            const float cT = hz_dv / T, cTn = hz_dv / Tn;                             // d v / d z at entry / exit
+            const float2 *Cu = C + (size_t)a * cplane + u;
+            const float *rsu = rs + (size_t)a * d.nv * d.nu + u;
+            float2 c1 = make_float2(0.f, 0.f);
+            float carry = 0.f;                         // moved into the row above by the rays crossing its lower plane
 #pragma unroll
-            for (int q = 0; q < KC; ++q) {
-                const int k = k0 + q;
-                if (k >= d.nz) break;
-                const float kf = (float)(k - d.koff);
-                const float sb = absdt_T * (fabsf(kf - d.zfrac) + 2.f) + 1e-3f;   // bound on |sz| near this row (+ slack)
-                const float zlo = kf - sb - d.zfrac, zhi = kf + 1.f + sb - d.zfrac;
-                const int vs = max(0, (int)ceilf(fmaf(zlo, invB, cv) - 1e-3f));
-                const int ve = min(d.nv - 1, (int)floorf(fmaf(zhi, invB, cv) + 1e-3f));
-                float s = 0.f;
-                for (int v = vs; v <= ve; ++v) {
-                    const float Za = z_entry(T, __ldg(d.zeta + v), d.zfrac);
-                    const float inv_sz = r.inv_dt * __ldg(d.inv_zeta + v);
-                    const float p0 = __saturatef((kf - Za) * inv_sz);
-                    const float p1 = __saturatef(((kf + 1.f) - Za) * inv_sz);
-                    const float w = fmaxf(0.f, fminf(l1, fmaxf(p0, p1)) - fmaxf(l0, fminf(p0, p1)));
-                    s = fmaf(w, __ldg(rsa + (size_t)v * d.nu), s);
+            for (int q = 0; q <= KC; ++q) {
+                // first ray at or above plane k0+q at the slab's entry / exit plane
+                const float zk = zk0 + (float)q;
+                const int vT = min(max((int)ceilf(fmaf(zk, cT, cv)), 0), d.nv);
+                const int vTn = min(max((int)ceilf(fmaf(zk, cTn, cv)), 0), d.nv);
+                const float2 c2 = __ldg(Cu + (size_t)vT * d.nu);
+                // rays crossing plane k0+q inside the slab: rising (entry row below the plane) if vTn < vT.
+                // The first one is evaluated unconditionally (weight 0 if there is none).
+                const int dlt = vTn - vT, vs = min(vT, vTn), vc = min(vs, d.nv - 1);
+                const float zkf = zk + d.zfrac;
+                const float bq = __saturatef((zkf - z_entry(T, __ldg(d.zeta + vc), d.zfrac)) * (r.inv_dt * __ldg(d.inv_zeta + vc)));
+                const float yq = __ldg(rsu + (size_t)vc * d.nu);
+                float up = fmaxf(0.f, l1 - fmaxf(l0, bq)) * (dlt < 0 ? yq : (dlt > 0 ? -yq : 0.f));   // moved up across the plane
+                if (abs(dlt) > 1) {                    // several rays cross this plane inside the slab (fine detector rows)
+                    for (int v = vs + 1; v < vs + abs(dlt); ++v) {
+                        const float b2 = __saturatef((zkf - z_entry(T, __ldg(d.zeta + v), d.zfrac)) * (r.inv_dt * __ldg(d.inv_zeta + v)));
+                        const float y2 = __ldg(rsu + (size_t)v * d.nu);
+                        up = fmaf(fmaxf(0.f, l1 - fmaxf(l0, b2)), dlt < 0 ? y2 : -y2, up);
+                    }
                 }
-                acc[q] += s;
+                if (q > 0) {
+                    const float ysum = (c2.x - c1.x) + (c2.y - c1.y);
+                    acc[q > 0 ? q - 1 : 0] += fmaf(w, ysum, carry - up);
+                }
+                c1 = c2;
+                carry = up;
             }
         }
     }
@@ -105,16 +163,30 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
     }
 }
 
+cbct_status op_backproject_prefix(cbct_geometry *g, const float *d_in, int scale, float *d_rs_out, cudaStream_t st)
+{
+    CBCT_TRY(ensure(g, &g->proj_prefix, (size_t)g->na * (g->nv + 1) * g->nu));
+    ProfileScope ps(2, st);
+    dim3 grid((g->nu + 127) / 128, g->na);
+    prefix_kernel<<<grid, 128, 0, st>>>(g->dev, d_in, scale, d_rs_out, g->proj_prefix);
+    CBCT_LAUNCH_CHECK();
+    return CBCT_OK;
+}
+
 cbct_status op_backproject_gather(cbct_geometry *g, const float *d_scaled, cudaStream_t st)
 {
-    constexpr int KC = 16, BI = 4;
+#ifndef CBCT_BP_KC
+#define CBCT_BP_KC 16
+#define CBCT_BP_BI 4
+#endif
+    constexpr int KC = CBCT_BP_KC, BI = CBCT_BP_BI;
     ProfileScope ps(3, st);
     for (int c = 0; c < 2; ++c) {
         if (g->n_tiles[c] == 0) continue;
         CBCT_TRY(ensure(g, &g->G_cls[c], g->n_vox()));
         const ClassGrid &cg = g->dev.cls[c];
         dim3 grid((cg.nmin + 31) / 32, (cg.nmaj + BI - 1) / BI, (g->nz + KC - 1) / KC), block(32, BI);
-        backproject_kernel<KC, BI><<<grid, block, 0, st>>>(g->dev, c, g->d_angle_has[c], d_scaled, g->G_cls[c]);
+        backproject_kernel<KC, BI><<<grid, block, 0, st>>>(g->dev, c, g->d_angle_has[c], d_scaled, g->proj_prefix, g->G_cls[c]);
         CBCT_LAUNCH_CHECK();
     }
     return CBCT_OK;

@@ -74,6 +74,7 @@ struct cbct_geometry {
     // lazily allocated scratch (device)
     float *vol_pad[2] = {nullptr, nullptr};   // padded [nz+2K][nmaj][row_stride] copies (class 0 transposed)
     float *proj_tmp = nullptr;                // scaled residual / projections
+    float2 *proj_prefix = nullptr;            // [na][nv+1][nu] compensated prefix sums of proj_tmp along v
     float *G_cls[2] = {nullptr, nullptr};     // per-class backprojection outputs (class 0 in [k][i][j] order)
     float *vol_a = nullptr, *vol_b = nullptr, *vol_c = nullptr, *vol_f = nullptr;   // g, u ping-pong, f
     float *Y_level = nullptr;                 // binned data for a coarse level
@@ -146,8 +147,10 @@ inline size_t pad_elems(const cbct_geometry *g, int c)
 cbct_status op_pad_copies(cbct_geometry *g, const float *d_vol, cudaStream_t st);
 // mode 0: out = P f ; mode 1: out = l * (P f - Y)  (scaled residual for the gather)
 cbct_status op_forward_padded(cbct_geometry *g, float *d_out, const float *d_Y, int mode, cudaStream_t st);
-cbct_status op_scale_proj(cbct_geometry *g, const float *d_proj, float *d_out, cudaStream_t st);
-// backprojector.cu : gathers of the (already l-scaled) projections into G_cls[0], G_cls[1]
+// backprojector.cu : gathers of the (already l-scaled) projections into G_cls[0], G_cls[1].
+// op_backproject_prefix builds the prefix sums along v that the gather reads (scale != 0: of l * d_in,
+// also written to d_rs_out); it must run on the same projections before op_backproject_gather.
+cbct_status op_backproject_prefix(cbct_geometry *g, const float *d_in, int scale, float *d_rs_out, cudaStream_t st);
 cbct_status op_backproject_gather(cbct_geometry *g, const float *d_scaled, cudaStream_t st);
 // out = G1 + G0^T                         (f == nullptr)
 // out = f - c (G1 + G0^T), optionally clamped at 0   (f != nullptr)

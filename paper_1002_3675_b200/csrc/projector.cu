@@ -184,23 +184,3 @@ cbct_status op_forward_padded(cbct_geometry *g, float *d_out, const float *d_Y, 
     }
     return CBCT_OK;
 }
-
-// scaled copy for the gather: out = l(u,v) * proj
-__global__ void __launch_bounds__(256) scale_proj_kernel(const DevGeom d, const float *__restrict__ in, float *__restrict__ out)
-{
-    const int u = blockIdx.x * blockDim.x + threadIdx.x;
-    const int v = blockIdx.y, a = blockIdx.z;
-    if (u >= d.nu) return;
-    const RayXY r = load_ray(d, a, u);
-    const size_t o = ((size_t)a * d.nv + v) * d.nu + u;
-    out[o] = chord_scale(r, __ldg(d.dz_mm + v)) * __ldg(in + o);
-}
-
-cbct_status op_scale_proj(cbct_geometry *g, const float *d_proj, float *d_out, cudaStream_t st)
-{
-    ProfileScope ps(2, st);
-    dim3 grid((g->nu + 255) / 256, g->nv, g->na);
-    scale_proj_kernel<<<grid, 256, 0, st>>>(g->dev, d_proj, d_out);
-    CBCT_LAUNCH_CHECK();
-    return CBCT_OK;
-}
