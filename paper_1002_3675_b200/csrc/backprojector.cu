@@ -123,6 +123,7 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
             const float cT = hz_dv / T, cTn = hz_dv / Tn;                             // d v / d z at entry / exit
             const float2 *Cu = C + (size_t)a * cplane + u;
             const float *rsu = rs + (size_t)a * d.nv * d.nu + u;
+            const float zkh1 = hz_dv * r.inv_dt, zkh0 = zk0 * zkh1, Tid = T * r.inv_dt;   // plane k0+q: zk hz/dv / dt = zkh0 + q zkh1
             float2 c1 = make_float2(0.f, 0.f);
             float carry = 0.f;                         // moved into the row above by the rays crossing its lower plane
 #pragma unroll
@@ -134,14 +135,17 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
                 const float2 c2 = __ldg(Cu + (size_t)vT * d.nu);
                 // rays crossing plane k0+q inside the slab: rising (entry row below the plane) if vTn < vT.
                 // The first one is evaluated unconditionally (weight 0 if there is none).
-                const int dlt = vTn - vT, vs = min(vT, vTn), vc = min(vs, d.nv - 1);
-                const float zkf = zk + d.zfrac;
-                const float bq = __saturatef((zkf - z_entry(T, __ldg(d.zeta + vc), d.zfrac)) * (r.inv_dt * __ldg(d.inv_zeta + vc)));
-                const float yq = __ldg(rsu + (size_t)vc * d.nu);
+                // b = lambda at which the ray meets the plane: T(lambda) zeta(v) = zk with T(lambda) = T + lambda dt and
+                // zeta(v) = (v - cv) dv / hz, i.e. b = (zk hz/dv / (v - cv) - T) / dt (the projector's b up to rounding;
+                // a ray in the central plane, v = cv, crosses nothing and the saturation turns its inf/NaN into 0 or 1).
+                const int dlt = vTn - vT, vs = min(vT, vTn);
+                const float zkh = zkh0 + (float)q * zkh1;
+                const float bq = __saturatef(__fdividef(zkh, (float)vs - cv) - Tid);
+                const float yq = __ldg(rsu + (size_t)min(vs, d.nv - 1) * d.nu);
                 float up = fmaxf(0.f, l1 - fmaxf(l0, bq)) * (dlt < 0 ? yq : (dlt > 0 ? -yq : 0.f));   // moved up across the plane
                 if (abs(dlt) > 1) {                    // several rays cross this plane inside the slab (fine detector rows)
                     for (int v = vs + 1; v < vs + abs(dlt); ++v) {
-                        const float b2 = __saturatef((zkf - z_entry(T, __ldg(d.zeta + v), d.zfrac)) * (r.inv_dt * __ldg(d.inv_zeta + v)));
+                        const float b2 = __saturatef(__fdividef(zkh, (float)v - cv) - Tid);
                         const float y2 = __ldg(rsu + (size_t)v * d.nu);
                         up = fmaf(fmaxf(0.f, l1 - fmaxf(l0, b2)), dlt < 0 ? y2 : -y2, up);
                     }
