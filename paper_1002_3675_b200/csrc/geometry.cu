@@ -99,6 +99,10 @@ static cbct_status build_tables(cbct_geometry *g)
         cg.joff = cg.nmin / 2;
         cg.row_stride = ((cg.nmin + kPadLo + kPadHi + 3) / 4) * 4;
         cg.plane_stride = (long long)cg.nmaj * cg.row_stride;
+        if ((long long)(g->nz + 2 * kPadK) * cg.plane_stride >= (1LL << 31)) {
+            cbct_set_error("geometry unsupported: the padded volume copy has 2^31 or more elements (32-bit offsets in the march)");
+            return CBCT_ERR_SHAPE;
+        }
     }
 
     std::vector<RayXY> rays((size_t)na * nu);

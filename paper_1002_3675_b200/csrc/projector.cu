@@ -100,22 +100,21 @@ forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, c
     if (lo_w < hi_w) {
         const float dirpos = r.sm >= 0.f ? 1.f : 0.f;
         const int dneg = r.sm >= 0.f ? 0 : 1;
-        float zeta[V], inv_sz[V], zbnd[V], zstep[V];
-        long long rowoff[V];
+        float zeta[V], inv_sz[V], zbnd[V];
+        int rowoff[V];                                          // element offsets fit 32 bits (checked at geometry creation)
+        const int pstride = (int)cg.plane_stride;
         const float e0 = (float)(lo_w - cg.ioff);
         const float T0 = fmaf(e0, r.dt, r.tc);
 #pragma unroll
         for (int q = 0; q < V; ++q) {
             const int v = min(v0 + q, d.nv - 1);
             zeta[q] = __ldg(d.zeta + v);
-            inv_sz[q] = r.inv_dt * __ldg(d.inv_zeta + v);
-            const float sz = r.dt * zeta[q];
-            zstep[q] = sz >= 0.f ? 1.f : -1.f;
+            inv_sz[q] = r.inv_dt * __ldg(d.inv_zeta + v);      // sign = direction of the ray in z
             const float Za = fmaf(T0, zeta[q], d.zfrac);
             const float kf = floorf(Za);
-            zbnd[q] = kf + (sz >= 0.f ? 1.f : 0.f);
+            zbnd[q] = kf + (inv_sz[q] >= 0.f ? 1.f : 0.f);
             const int k = (int)kf + d.koff;
-            rowoff[q] = (long long)(min(max(k, -kPadK), d.nz + kPadK - 1) + kPadK) * cg.plane_stride;
+            rowoff[q] = (min(max(k, -kPadK), d.nz + kPadK - 1) + kPadK) * pstride;
         }
         const float *base = vol + kPadLo;
         for (int i = lo_w; i < hi_w; ++i) {
@@ -128,30 +127,33 @@ forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, c
             const float oma = 1.f - a_;
             const float wlo = dneg ? oma : a_;                 // fraction [0,a] belongs to row ja, [a,1] to ja+dir
             const float whi = dneg ? a_ : oma;
-            const long long off_i = (long long)i * cg.row_stride + jlo;
+            const int off_i = i * cg.row_stride + jlo;
+            // Pass 1, branch-free: every ray as if it stayed in its entry z row for the whole slab
+            // (all 2V loads are independent and in flight together).
+            float b[V];
 #pragma unroll
             for (int q = 0; q < V; ++q) {
                 const float Za = fmaf(T, zeta[q], d.zfrac);
-                const float b = __saturatef((zbnd[q] - Za) * inv_sz[q]);
-                const float *p = base + rowoff[q] + off_i;
-                if (!__any_sync(0xffffffffu, b < 1.f)) {
-                    acc[q] = fmaf(wlo, __ldg(p), acc[q]);
-                    acc[q] = fmaf(whi, __ldg(p + 1), acc[q]);
-                } else {
-                    // z-plane crossing inside this slab for some lane: general four-term form
-                    const int k1 = (int)(zbnd[q] - (zstep[q] > 0.f ? 1.f : 0.f) + zstep[q]) + d.koff;
-                    const long long rowoff1 = (long long)(min(max(k1, -kPadK), d.nz + kPadK - 1) + kPadK) * cg.plane_stride;
-                    const float *p1 = base + rowoff1 + off_i;
-                    const float mn = fminf(a_, b), mx = fmaxf(a_, b);
-                    const float w_r0k0 = mn, w_r1k0 = b - mn, w_r0k1 = a_ - mn, w_r1k1 = 1.f - mx;
-                    const float wl0 = dneg ? w_r1k0 : w_r0k0, wh0 = dneg ? w_r0k0 : w_r1k0;
-                    const float wl1 = dneg ? w_r1k1 : w_r0k1, wh1 = dneg ? w_r0k1 : w_r1k1;
-                    float s = wl0 * __ldg(p);
-                    s = fmaf(wh0, __ldg(p + 1), s);
-                    s = fmaf(wl1, __ldg(p1), s);
-                    s = fmaf(wh1, __ldg(p1 + 1), s);
-                    acc[q] += s;
-                    if (b < 1.f) { zbnd[q] += zstep[q]; rowoff[q] = rowoff1; }
+                b[q] = __saturatef((zbnd[q] - Za) * inv_sz[q]);
+                const float *p = base + (rowoff[q] + off_i);
+                acc[q] = fmaf(wlo, __ldg(p), acc[q]);
+                acc[q] = fmaf(whi, __ldg(p + 1), acc[q]);
+            }
+            // Pass 2: a ray that crosses a z plane inside the slab (b < 1) moves its exit-row fractions
+            // a - min(a,b) (row ja) and 1 - max(a,b) (row ja+dir) to the next z row, and continues there.
+#pragma unroll
+            for (int q = 0; q < V; ++q) {
+                if (b[q] < 1.f) {
+                    const float zs = inv_sz[q] >= 0.f ? 1.f : -1.f;
+                    const int k1 = (int)(zbnd[q] - (zs > 0.f ? 1.f : 0.f) + zs) + d.koff;
+                    const int rowoff1 = (min(max(k1, -kPadK), d.nz + kPadK - 1) + kPadK) * pstride;
+                    const float *p = base + (rowoff[q] + off_i), *p1 = base + (rowoff1 + off_i);
+                    const float c_r0 = a_ - fminf(a_, b[q]), c_r1 = 1.f - fmaxf(a_, b[q]);
+                    const float c_lo = dneg ? c_r1 : c_r0, c_hi = dneg ? c_r0 : c_r1;
+                    acc[q] = fmaf(c_lo, __ldg(p1) - __ldg(p), acc[q]);
+                    acc[q] = fmaf(c_hi, __ldg(p1 + 1) - __ldg(p + 1), acc[q]);
+                    zbnd[q] += zs;
+                    rowoff[q] = rowoff1;
                 }
             }
         }
