@@ -174,7 +174,11 @@ forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, c
 
 cbct_status op_forward_padded(cbct_geometry *g, float *d_out, const float *d_Y, int mode, cudaStream_t st)
 {
-    constexpr int V = 8, WARPS = 4;
+#ifndef CBCT_FW_V
+#define CBCT_FW_V 4
+#define CBCT_FW_WARPS 4
+#endif
+    constexpr int V = CBCT_FW_V, WARPS = CBCT_FW_WARPS;
     ProfileScope ps(1, st);
     // rays in no tile miss the volume: P f = 0 there
     if (mode == 0) CBCT_CUDA(cudaMemsetAsync(d_out, 0, g->n_proj() * sizeof(float), st));
