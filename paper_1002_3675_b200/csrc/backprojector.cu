@@ -133,21 +133,24 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
                 const int vT = min(max((int)ceilf(fmaf(zk, cT, cv)), 0), d.nv);
                 const int vTn = min(max((int)ceilf(fmaf(zk, cTn, cv)), 0), d.nv);
                 const float2 c2 = __ldg(Cu + (size_t)vT * d.nu);
-                // rays crossing plane k0+q inside the slab: rising (entry row below the plane) if vTn < vT.
-                // The first one is evaluated unconditionally (weight 0 if there is none).
+                // rays crossing plane k0+q inside the slab: v in [min(vT,vTn), max(vT,vTn)).  The arithmetic of the first
+                // one runs unconditionally (its y is 0 if there is none).
                 // b = lambda at which the ray meets the plane: T(lambda) zeta(v) = zk with T(lambda) = T + lambda dt and
                 // zeta(v) = (v - cv) dv / hz, i.e. b = (zk hz/dv / (v - cv) - T) / dt (the projector's b up to rounding;
                 // a ray in the central plane, v = cv, crosses nothing and the saturation turns its inf/NaN into 0 or 1).
                 const int dlt = vTn - vT, vs = min(vT, vTn);
                 const float zkh = zkh0 + (float)q * zkh1;
                 const float bq = __saturatef(__fdividef(zkh, (float)vs - cv) - Tid);
-                const float yq = __ldg(rsu + (size_t)min(vs, d.nv - 1) * d.nu);
-                float up = fmaxf(0.f, l1 - fmaxf(l0, bq)) * (dlt < 0 ? yq : (dlt > 0 ? -yq : 0.f));   // moved up across the plane
+                // rising iff dt zeta > 0, and zkh = zk hz/dv / dt has that sign for the rays near plane zk: move its sign bit onto y
+                float yq = 0.f;
+                if (dlt != 0) yq = __ldg(rsu + (size_t)vs * d.nu);
+                yq = __int_as_float(__float_as_int(yq) ^ (__float_as_int(zkh) & 0x80000000));
+                float up = fmaxf(0.f, l1 - fmaxf(l0, bq)) * yq;       // moved up across the plane (negative: moved down)
                 if (abs(dlt) > 1) {                    // several rays cross this plane inside the slab (fine detector rows)
                     for (int v = vs + 1; v < vs + abs(dlt); ++v) {
                         const float b2 = __saturatef(__fdividef(zkh, (float)v - cv) - Tid);
                         const float y2 = __ldg(rsu + (size_t)v * d.nu);
-                        up = fmaf(fmaxf(0.f, l1 - fmaxf(l0, b2)), dlt < 0 ? y2 : -y2, up);
+                        up = fmaf(fmaxf(0.f, l1 - fmaxf(l0, b2)), __int_as_float(__float_as_int(y2) ^ (__float_as_int(zkh) & 0x80000000)), up);
                     }
                 }
                 if (q > 0) {
