@@ -151,6 +151,9 @@ cbct_status op_tv_sweep(cbct_geometry *g, const float *u_in, const float *gv, fl
                         float beta, float eps, float dt, int clamp, cudaStream_t st)
 {
     ProfileScope ps(5, st);
+    int done = 0;
+    CBCT_TRY(op_tv_sweep_rows(g, u_in, gv, u_out, beta, eps, dt, clamp, st, &done));   // nx <= 512: row-streaming kernel (tv_rows.cu)
+    if (done) return CBCT_OK;
     dim3 grid((g->nx + TX - 1) / TX, (g->ny + TY - 1) / TY, (g->nz + TZ - 1) / TZ);
     const int vec_ok = (g->nx % 4 == 0) && ((reinterpret_cast<uintptr_t>(u_in) & 15) == 0);
     tv_sweep_kernel<<<grid, 256, 0, st>>>(u_in, gv, u_out, g->nx, g->ny, g->nz, (float)(1.0 / g->hx),
