@@ -87,7 +87,7 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
     const float ef = (float)(i - cg.ioff);
     const float cu = 0.5f * (float)(d.nu - 1), cv = 0.5f * (float)(d.nv - 1);
     const float sdd_du = d.sdd / d.du;
-    const float hz_dv = d.hz / d.dv;
+    const float hz_dv = d.hz / d.dv, dv_hz = d.dv / d.hz;
     const float zk0 = (float)(k0 - d.koff) - d.zfrac;  // plane k0 in the units of z_entry(), minus zfrac
     const size_t cplane = (size_t)(d.nv + 1) * d.nu;
 
@@ -123,7 +123,7 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
             const float cT = hz_dv / T, cTn = hz_dv / Tn;                             // d v / d z at entry / exit
             const float2 *Cu = C + (size_t)a * cplane + u;
             const float *rsu = rs + (size_t)a * d.nv * d.nu + u;
-            const float zkh1 = hz_dv * r.inv_dt, zkh0 = zk0 * zkh1, Tid = T * r.inv_dt;   // plane k0+q: zk hz/dv / dt = zkh0 + q zkh1
+            const float Tdv = T * dv_hz, dtdv = r.dt * dv_hz;                         // T zeta(v) = Tdv (v - cv), dt zeta(v) = dtdv (v - cv)
             float2 c1 = make_float2(0.f, 0.f);
             float carry = 0.f;                         // moved into the row above by the rays crossing its lower plane
 #pragma unroll
@@ -136,21 +136,21 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
                 // rays crossing plane k0+q inside the slab: v in [min(vT,vTn), max(vT,vTn)).  The arithmetic of the first
                 // one runs unconditionally (its y is 0 if there is none).
                 // b = lambda at which the ray meets the plane: T(lambda) zeta(v) = zk with T(lambda) = T + lambda dt and
-                // zeta(v) = (v - cv) dv / hz, i.e. b = (zk hz/dv / (v - cv) - T) / dt (the projector's b up to rounding;
-                // a ray in the central plane, v = cv, crosses nothing and the saturation turns its inf/NaN into 0 or 1).
+                // zeta(v) = (v - cv) dv / hz, i.e. b = (zk - T zeta(v)) / (dt zeta(v)), the projector's b with its numerator
+                // taken by one FMA (a ray in the central plane, v = cv, crosses nothing; saturation turns its 0/0 into 0).
                 const int dlt = vTn - vT, vs = min(vT, vTn);
-                const float zkh = zkh0 + (float)q * zkh1;
-                const float bq = __saturatef(__fdividef(zkh, (float)vs - cv) - Tid);
-                // rising iff dt zeta > 0, and zkh = zk hz/dv / dt has that sign for the rays near plane zk: move its sign bit onto y
+                const float vf = (float)vs - cv;
+                const float bq = __saturatef(__fdividef(fmaf(-Tdv, vf, zk), vf * dtdv));
+                // rising iff dt zeta(v) > 0: move the sign bit of dt zeta(v) onto y
                 float yq = 0.f;
                 if (dlt != 0) yq = __ldg(rsu + (size_t)vs * d.nu);
-                yq = __int_as_float(__float_as_int(yq) ^ (__float_as_int(zkh) & 0x80000000));
+                yq = __int_as_float(__float_as_int(yq) ^ (__float_as_int(vf * dtdv) & 0x80000000));
                 float up = fmaxf(0.f, l1 - fmaxf(l0, bq)) * yq;       // moved up across the plane (negative: moved down)
                 if (abs(dlt) > 1) {                    // several rays cross this plane inside the slab (fine detector rows)
                     for (int v = vs + 1; v < vs + abs(dlt); ++v) {
-                        const float b2 = __saturatef(__fdividef(zkh, (float)v - cv) - Tid);
+                        const float b2 = __saturatef(__fdividef(fmaf(-Tdv, (float)v - cv, zk), ((float)v - cv) * dtdv));
                         const float y2 = __ldg(rsu + (size_t)v * d.nu);
-                        up = fmaf(fmaxf(0.f, l1 - fmaxf(l0, b2)), __int_as_float(__float_as_int(y2) ^ (__float_as_int(zkh) & 0x80000000)), up);
+                        up = fmaf(fmaxf(0.f, l1 - fmaxf(l0, b2)), __int_as_float(__float_as_int(y2) ^ (__float_as_int(vf * dtdv) & 0x80000000)), up);
                     }
                 }
                 if (q > 0) {
