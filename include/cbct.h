@@ -168,7 +168,7 @@ cbct_status cbct_fbs_reconstruct_host(const cbct_geometry *g, const float *h_Y, 
 
 /*
  * Per-kernel-class device timing (CUDA events recorded around each launch on the launching stream).
- * Classes: 0 pad/transposed volume copies, 1 forward projector, 2 projection scaling, 3 backprojector
+ * Classes: 0 pad/transposed volume copies, 1 forward projector, 2 projection scaling + prefix sums along v, 3 backprojector
  * gather, 4 combine / gradient step, 5 TV sweep, 6 multigrid transfers, 7 reductions.
  * cbct_profile_read fills h_ms[CBCT_PROFILE_TAGS] (summed milliseconds) and h_count[] (launch groups)
  * since the last reset; it waits for the recorded events.  Off by default.

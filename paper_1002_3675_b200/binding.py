@@ -78,7 +78,7 @@ def launch_count() -> int:
     return int(load().cbct_launch_count())
 
 
-PROFILE_TAGS = ("pad_copy", "forward", "scale_proj", "backproject", "combine", "tv_sweep", "transfers", "reductions")
+PROFILE_TAGS = ("pad_copy", "forward", "proj_prefix", "backproject", "combine", "tv_sweep", "transfers", "reductions")
 
 
 def profile_enable(on: bool):
