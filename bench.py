@@ -239,10 +239,13 @@ def run_gpu(args):
     nnz_fine = float(frozen("nnz", "c2", NNZ["c2"]))
     nnz_step = nnz_fine * (1.0 + frozen("nnz_coarse_ratio", "c2", 0.125))
     sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
-    traffic = None
+    traffic = None                      # DRAM bytes per launch of that kernel from the committed ncu capture (profiles/traffic.csv)
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
-            traffic = json.load(fh).get(dom)
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as fh:
+            for line in fh.read().splitlines()[1:]:
+                k, v = line.split(",")[:2]
+                if k == dom:
+                    traffic = float(v)
     except Exception:
         pass
     if dom == "tv_sweep":
