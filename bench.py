@@ -122,6 +122,21 @@ def level_dims(g, levels):
     return out
 
 
+def max_over_ranks(seconds: float, dist, device) -> float:
+    """Whole-job time of a replicas-only run: the slowest rank's device-timed seconds (all-reduce MAX)."""
+    if dist is None:
+        return float(seconds)
+    import torch
+    t = torch.tensor([seconds], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, updates_per_step: float, steps: int, seconds: float) -> float:
+    """Aggregate GUPS over all ranks: every rank processed `updates_per_step` per step (weak scaling)."""
+    return world * updates_per_step * steps / seconds / 1e9
+
+
 def run_gpu(args):
     import torch
     import paper_1002_3675_b200 as cb
@@ -190,11 +205,7 @@ def run_gpu(args):
     prof = cb.profile_read(reset=True)
     cb.profile_enable(False)
     ms = [a.elapsed_time(b) for a, b in ev]
-    t_total = sum(ms) / 1e3
-    if dist is not None:
-        t = torch.tensor([t_total], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        t_total = float(t.item())
+    t_total = max_over_ranks(sum(ms) / 1e3, dist, dev)
 
     # ---- end-to-end: host buffers through the C ABI, copies inside the timed region ----
     h_f.copy_(d_f.cpu())
@@ -209,11 +220,7 @@ def run_gpu(args):
             step_host()
             b.record(st)
     barrier()
-    t_e2e = sum(a.elapsed_time(b) for a, b in ev2) / 1e3
-    if dist is not None:
-        t = torch.tensor([t_e2e], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        t_e2e = float(t.item())
+    t_e2e = max_over_ranks(sum(a.elapsed_time(b) for a, b in ev2) / 1e3, dist, dev)
 
     if rank != 0:
         if dist is not None:
@@ -222,8 +229,8 @@ def run_gpu(args):
 
     pk = peaks()
     K = args.steps
-    value = world * updates * K / t_total / 1e9
-    e2e_value = world * updates * K / t_e2e / 1e9
+    value = whole_job_value(world, updates, K, t_total)
+    e2e_value = whole_job_value(world, updates, K, t_e2e)
 
     # per-operator numbers from the live per-class event timing (fine + coarse level launches summed)
     def per_step_ms(tag):
