@@ -44,6 +44,8 @@ def lib():
         L.oracle_backproject.argtypes = [gp, dp, dp]
         L.oracle_backproject.restype = C.c_int
         L.oracle_backproject_voxels.argtypes = [gp, dp, C.c_long, ip, ip, ip, dp]
+        L.oracle_backproject_eq2.argtypes = [gp, dp, dp]
+        L.oracle_backproject_eq2.restype = None
         d, i = C.c_double, C.c_int
         L.oracle_tv_value.argtypes = [dp, i, i, i, d, d, d, d]
         L.oracle_tv_value.restype = d
@@ -127,6 +129,16 @@ def backproject_voxels(g, proj, ix, iy, iz) -> np.ndarray:
     out = np.empty(ix.shape[0])
     gs = _geom(g)
     lib().oracle_backproject_voxels(C.byref(gs), _dptr(proj), ix.shape[0], _iptr(ix), _iptr(iy), _iptr(iz), _dptr(out))
+    return out
+
+
+def backproject_eq2(g, proj) -> np.ndarray:
+    """Eq. 2 without its prefactor 2/(N_theta A):
+    (B r)(x) = sum_theta L^3(u*,v*) / (L0 l^2(x)) r(u*,v*), bilinear r, zero outside the detector (Q4)."""
+    proj = _proj(g, proj)
+    out = np.empty(g.vol_shape)
+    gs = _geom(g)
+    lib().oracle_backproject_eq2(C.byref(gs), _dptr(proj), _dptr(out))
     return out
 
 

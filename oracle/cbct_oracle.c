@@ -15,10 +15,14 @@
  *   O2 backprojector   P:95  "P^T denotes a matrix transpose": literal scatter of O1
  *   O3/O4 TV           P:69 E1 = (1/V)||grad f||_1, smoothed by eps (Q6); P:93 gradient descent
  *
+ *   NEXT-1 eq. 2     P:97-99  the paper's voxel-driven backprojector (oracle_backproject_eq2)
+ *
  * Pins (tests/test_oracle_*.py): closed-form box chord (I1), brute-force dense matrix
  * on 8^3 and 6x8x4 (I2), analytic ellipsoid chords (I3), dot-product identity (I4), eq. 2
  * weight (I5), rot90 / z-flip symmetry (I6), TV invariants + finite differences (I7),
- * descent (I8, I9), dense-matrix FBS (I10), NNLS limit (I11), transfer identities (I12).
+ * descent (I8, I9), dense-matrix FBS (I10), NNLS limit (I11), transfer identities (I12);
+ * eq. 2: hand-worked weights and interpolation, a library interpolation routine on a tiny case,
+ * convergence to (du dv / dV) P^T under refinement (test_oracle_eq2.py).
  * Parity unpinned BY THE PAPER (fixed by DESIGN.md, identical on both sides): the choice of
  * eps, omega, u0, the coarsening rule and prolongation weights (those live in fbs.py).
  */
@@ -332,6 +336,58 @@ void oracle_backproject_voxels(const og_geom *g, const double *proj, long n,
                 }
         }
         out[q] = acc;
+    }
+}
+
+/*
+ * NEXT-1: the paper's own voxel-driven backprojector, eq. 2, without the prefactor
+ * 2/(N_theta A) (applied by the caller):
+ *   (B r)(x) = sum_theta  L^3(u*,v*) / (L0 l^2(x)) * r^theta(u*,v*)
+ * x the voxel centre; (u*,v*) where the line source -> x meets the imager; L0 the source-imager
+ * distance; l = |x - S|; L = |(u*,v*) - S|.  r at (u*,v*) by bilinear interpolation between
+ * pixel centres, r = 0 outside the detector (reading Q4).  Not the transpose of O1; it agrees with
+ * (du dv / dV) P^T r as the grids are refined (pinned in tests/test_oracle_eq2.py).
+ */
+void oracle_backproject_eq2(const og_geom *g, const double *proj, double *vol)
+{
+    const double L0 = g->sdd;
+#pragma omp parallel for schedule(static)
+    for (long kj = 0; kj < (long)g->nz * g->ny; ++kj) {
+        int k = (int)(kj / g->ny), j = (int)(kj % g->ny);
+        for (int i = 0; i < g->nx; ++i) {
+            double x[3] = {((double)i - 0.5 * (g->nx - 1)) * g->hx, ((double)j - 0.5 * (g->ny - 1)) * g->hy,
+                           ((double)k - 0.5 * (g->nz - 1)) * g->hz};
+            double acc = 0.0;
+            for (int ia = 0; ia < g->n_angles; ++ia) {
+                double t = g->angles[ia], c = cos(t), s = sin(t);
+                double S[3] = {g->sad * c, g->sad * s, 0.0};
+                double Cd[3] = {-(g->sdd - g->sad) * c, -(g->sdd - g->sad) * s, 0.0};   /* imager centre */
+                double n[3] = {-c, -s, 0.0};                                             /* source -> imager normal */
+                double uh[3] = {-s, c, 0.0}, vh[3] = {0.0, 0.0, 1.0};                    /* imager axes */
+                double dxs[3] = {x[0] - S[0], x[1] - S[1], x[2] - S[2]};
+                double depth = dxs[0] * n[0] + dxs[1] * n[1] + dxs[2] * n[2];
+                if (depth <= 0.0) continue;
+                double tau = L0 / depth;                                                 /* S + tau (x - S) lies on the imager */
+                double Pt[3] = {S[0] + tau * dxs[0], S[1] + tau * dxs[1], S[2] + tau * dxs[2]};
+                double ustar = (Pt[0] - Cd[0]) * uh[0] + (Pt[1] - Cd[1]) * uh[1] + (Pt[2] - Cd[2]) * uh[2];
+                double vstar = (Pt[0] - Cd[0]) * vh[0] + (Pt[1] - Cd[1]) * vh[1] + (Pt[2] - Cd[2]) * vh[2];
+                double l = sqrt(dxs[0] * dxs[0] + dxs[1] * dxs[1] + dxs[2] * dxs[2]);
+                double L = sqrt((Pt[0] - S[0]) * (Pt[0] - S[0]) + (Pt[1] - S[1]) * (Pt[1] - S[1]) + (Pt[2] - S[2]) * (Pt[2] - S[2]));
+                double pu = ustar / g->du + 0.5 * (g->nu - 1), pv = vstar / g->dv + 0.5 * (g->nv - 1);
+                double fu = floor(pu), fv = floor(pv);
+                int iu = (int)fu, iv = (int)fv;
+                double au = pu - fu, av = pv - fv, val = 0.0;
+                const double *img = proj + (size_t)ia * g->nv * g->nu;
+                for (int dv_ = 0; dv_ < 2; ++dv_)
+                    for (int du_ = 0; du_ < 2; ++du_) {
+                        int uu = iu + du_, vv = iv + dv_;
+                        if (uu < 0 || uu >= g->nu || vv < 0 || vv >= g->nv) continue;
+                        val += (du_ ? au : 1.0 - au) * (dv_ ? av : 1.0 - av) * img[(size_t)vv * g->nu + uu];
+                    }
+                acc += L * L * L / (L0 * l * l) * val;
+            }
+            vol[((size_t)k * g->ny + j) * g->nx + i] = acc;
+        }
     }
 }
 

@@ -42,14 +42,20 @@ def energy(g, f, Y, mu: float, eps: float, Pf: Optional[np.ndarray] = None) -> d
 # ----------------------------------------------------------------------------------------
 def fbs_level(g, Y, f0, n_outer: int, n_inner: int, step: float, mu: float, eps: float,
               omega: float = 1.0, u0_mode: str = "g", clamp: bool = True,
-              trace: Optional[list] = None) -> np.ndarray:
+              trace: Optional[list] = None, backprojector: str = "exact") -> np.ndarray:
+    """backprojector = "exact": dE2/df through the matrix transpose (P:95, the hot path);
+    "eq2": through the paper's eq. 2: dE2/df(x) = (2/(N_theta A)) (B r)(x), so step 1 reads
+    g = f - (mu V/beta) dE2/df = f - c (dV/(du dv)) (B r) with the same c."""
     o = _prims()
     f = np.array(f0, dtype=np.float64, copy=True)
     beta = mu / step
     c = 2.0 * step * g.n_vox / (g.n_angles * g.n_pix)
     for _ in range(n_outer):
         r = o.forward(g, f) - Y                      # P f - Y            (P:99)
-        G = o.backproject(g, r)                      # P^T (P f - Y)
+        if backprojector == "exact":
+            G = o.backproject(g, r)                  # P^T (P f - Y)      (P:95)
+        else:
+            G = (g.hx * g.hy * g.hz / (g.du * g.dv)) * o.backproject_eq2(g, r)   # eq. 2 (P:97)
         gv = f - c * G                               # step 1             (P:87)
         u0 = gv if u0_mode == "g" else f             # Q7: start of the inner descent
         u = o.tv_prox(g, gv, u0, beta, eps, omega, n_inner)   # step 2    (P:89, P:93)
@@ -144,7 +150,7 @@ def prolong(c: np.ndarray, axes) -> np.ndarray:
 
 def fbs_reconstruct(g, Y, f0, n_levels: int, n_outer: Sequence[int], n_inner: int, step: float,
                     mu: float, eps: float, omega: float = 1.0, u0_mode: str = "g",
-                    clamp: bool = True, trace: Optional[list] = None) -> np.ndarray:
+                    clamp: bool = True, trace: Optional[list] = None, backprojector: str = "exact") -> np.ndarray:
     """O6: run O5 at the coarsest level from f0 (zeros if None; a caller's fine-grid f0 is
     restricted down), prolong to the next level, repeat; n_outer is listed coarsest first.
     n_levels = 1 is exactly O5."""
@@ -161,7 +167,7 @@ def fbs_reconstruct(g, Y, f0, n_levels: int, n_outer: Sequence[int], n_inner: in
             f = restrict_volume(f, ax)
     for n, lev in enumerate(range(n_levels - 1, -1, -1)):
         f = fbs_level(geoms[lev], Ys[lev], f, n_outer[n], n_inner, step, mu, eps, omega,
-                      u0_mode=u0_mode, clamp=clamp, trace=trace)
+                      u0_mode=u0_mode, clamp=clamp, trace=trace, backprojector=backprojector)
         if lev > 0:
             f = prolong(f, axes[lev - 1])
     return f

@@ -122,3 +122,27 @@ def dense_fbs(A, g, Y, f0, n_outer, n_inner, step, mu, eps, omega=1.0, u0_mode="
         f = np.maximum(u, 0.0) if clamp else u
         its.append(f.reshape(g.vol_shape).copy())
     return its
+
+
+def eq2_backproject(g, r):
+    """Eq. 2 a second time, from similar triangles instead of 3-D distances, with the
+    interpolation done by a library routine (scipy.ndimage.map_coordinates, order 1, zero beyond the grid):
+    voxel centre x; t = depth of x along the central ray, s = lateral offset; u* = SDD s/t, v* = SDD z/t;
+    L/l = SDD/t  =>  L^3/(L0 l^2) = (SDD/t)^2 (l/t)."""
+    from scipy.ndimage import map_coordinates
+    xs = (np.arange(g.nx) - (g.nx - 1) / 2.0) * g.hx
+    ys = (np.arange(g.ny) - (g.ny - 1) / 2.0) * g.hy
+    zs = (np.arange(g.nz) - (g.nz - 1) / 2.0) * g.hz
+    Z, Y, X = np.meshgrid(zs, ys, xs, indexing="ij")
+    out = np.zeros(g.vol_shape)
+    for ia, th in enumerate(np.asarray(g.angles)):
+        c, s = np.cos(th), np.sin(th)
+        t = g.sad - (X * c + Y * s)
+        lat = -X * s + Y * c
+        pu = g.sdd * lat / t / g.du + (g.nu - 1) / 2.0
+        pv = g.sdd * Z / t / g.dv + (g.nv - 1) / 2.0
+        val = map_coordinates(np.asarray(r[ia], dtype=np.float64), [pv.ravel(), pu.ravel()], order=1,
+                              mode="grid-constant", cval=0.0).reshape(g.vol_shape)
+        w = (g.sdd / t) ** 2 * np.sqrt(t * t + lat * lat + Z * Z) / t
+        out += w * val
+    return out
