@@ -95,6 +95,25 @@ cbct_status cbct_forward(const cbct_geometry *g, const float *d_vol, float *d_pr
 cbct_status cbct_backproject(const cbct_geometry *g, const float *d_proj, float *d_vol, void *cuda_stream);
 
 /*
+ * NEXT-1. The paper's own voxel-driven backprojector, eq. 2, without its prefactor 2/(N_theta A):
+ *   (B r)(x) = sum_theta L^3(u*,v*) / (L0 l^2(x)) r(u*,v*)
+ * x the voxel centre, (u*,v*) where the line source -> x meets the imager, L0 = sdd, l = |x - S|,
+ * L = |(u*,v*) - S|; r is interpolated bilinearly between pixel centres and is 0 outside the detector.
+ * It is NOT the transpose of cbct_forward; (du dv / dV) P^T r tends to B r as the grids are refined.
+ * d_vol is overwritten.
+ */
+cbct_status cbct_backproject_eq2(const cbct_geometry *g, const float *d_proj, float *d_vol, void *cuda_stream);
+
+/*
+ * Which backprojector step 1 of cbct_fbs_reconstruct uses: the exact transpose (default; the path
+ * BASELINE.json's north_star names) or eq. 2 as the paper ran it, g = f - (mu V / beta) (2/(N_theta A)) B r.
+ * Applies to this handle and the coarse levels of its cascades.  Errors: INVALID_ARG for another value.
+ */
+#define CBCT_BACKPROJECTOR_EXACT 0
+#define CBCT_BACKPROJECTOR_EQ2 1
+cbct_status cbct_set_backprojector(cbct_geometry *g, int mode);
+
+/*
  * a5. TV-prox inner descent (P:89 step 2, "solved by a simple gradient descent method"; O4):
  * n_inner Jacobi steps  u <- u - dt [ beta (u - g) + grad TV_eps(u) ],
  *   dt = omega / (beta + 4 (1/hx^2 + 1/hy^2 + 1/hz^2) / eps),

@@ -15,7 +15,7 @@ STATUS = {0: "CBCT_OK", 1: "CBCT_ERR_INVALID_ARG", 2: "CBCT_ERR_SHAPE", 3: "CBCT
 # every symbol include/cbct.h declares (tests check that the library exports each of them)
 SYMBOLS = (
     "cbct_geometry_create", "cbct_geometry_destroy", "cbct_geometry_query", "cbct_geometry_coarsen",
-    "cbct_forward", "cbct_backproject", "cbct_tv_prox", "cbct_prolong", "cbct_restrict", "cbct_bin2x2",
+    "cbct_forward", "cbct_backproject", "cbct_backproject_eq2", "cbct_set_backprojector", "cbct_tv_prox", "cbct_prolong", "cbct_restrict", "cbct_bin2x2",
     "cbct_energy", "cbct_fbs_reconstruct", "cbct_forward_host", "cbct_backproject_host", "cbct_tv_prox_host",
     "cbct_fbs_reconstruct_host", "cbct_profile_enable", "cbct_profile_read", "cbct_launch_count", "cbct_device_bytes", "cbct_last_error",
 )
@@ -49,6 +49,8 @@ def load():
     L.cbct_geometry_coarsen.argtypes = [vp, C.POINTER(vp), ip]
     L.cbct_forward.argtypes = [vp, fp, fp, vp]
     L.cbct_backproject.argtypes = [vp, fp, fp, vp]
+    L.cbct_backproject_eq2.argtypes = [vp, fp, fp, vp]
+    L.cbct_set_backprojector.argtypes = [vp, i]
     L.cbct_tv_prox.argtypes = [vp, fp, fp, f, f, f, i, vp]
     L.cbct_prolong.argtypes = [vp, fp, fp, vp]
     L.cbct_restrict.argtypes = [vp, fp, fp, vp]
@@ -197,6 +199,19 @@ def forward(g: Geometry, d_vol, d_proj, stream=None):
 
 def backproject(g: Geometry, d_proj, d_vol, stream=None):
     _check(load().cbct_backproject(g._h, _dev(d_proj, g.n_proj, "d_proj"), _dev(d_vol, g.n_vox, "d_vol"), _stream(stream)))
+
+
+def backproject_eq2(g: Geometry, d_proj, d_vol, stream=None):
+    """The paper's eq. 2 backprojector without its prefactor; not the transpose of forward()."""
+    _check(load().cbct_backproject_eq2(g._h, _dev(d_proj, g.n_proj, "d_proj"), _dev(d_vol, g.n_vox, "d_vol"), _stream(stream)))
+
+
+BACKPROJECTOR_EXACT, BACKPROJECTOR_EQ2 = 0, 1
+
+
+def set_backprojector(g: Geometry, mode: int):
+    """Backprojector of step 1 in fbs_reconstruct: BACKPROJECTOR_EXACT (default) or BACKPROJECTOR_EQ2."""
+    _check(load().cbct_set_backprojector(g._h, int(mode)))
 
 
 def tv_prox(g: Geometry, d_g, d_u, beta, eps, omega, n_inner, stream=None):

@@ -36,6 +36,20 @@ extern "C" cbct_status cbct_backproject(const cbct_geometry *gc, const float *d_
     return op_combine(g, nullptr, 0.f, 0, d_vol, st);
 }
 
+extern "C" cbct_status cbct_backproject_eq2(const cbct_geometry *gc, const float *d_proj, float *d_vol, void *stream)
+{
+    REQUIRE(gc && d_proj && d_vol, "cbct_backproject_eq2: NULL argument");
+    return op_backproject_eq2(mut(gc), d_proj, nullptr, 0.f, 0, d_vol, (cudaStream_t)stream);
+}
+
+extern "C" cbct_status cbct_set_backprojector(cbct_geometry *g, int mode)
+{
+    REQUIRE(g, "cbct_set_backprojector: NULL handle");
+    REQUIRE(mode == CBCT_BACKPROJECTOR_EXACT || mode == CBCT_BACKPROJECTOR_EQ2, "cbct_set_backprojector: unknown mode %d", mode);
+    g->bp_mode = mode;
+    return CBCT_OK;
+}
+
 static float tv_dt(const cbct_geometry *g, float beta, float eps, float omega)
 {
     const double K = 4.0 * (1.0 / (g->hx * g->hx) + 1.0 / (g->hy * g->hy) + 1.0 / (g->hz * g->hz));
@@ -131,15 +145,28 @@ static cbct_status fbs_level(cbct_geometry *g, const float *d_Y, float *f, int n
     const float c = (float)(2.0 * (double)step * (double)g->n_vox() / ((double)g->na * g->nu * g->nv));
     for (int it = 0; it < n_outer; ++it) {
         CBCT_TRY(op_pad_copies(g, f, st));
-        CBCT_TRY(op_forward_padded(g, g->proj_tmp, d_Y, 1, st));          // l (P f - Y)          a1+a2
-        CBCT_TRY(op_backproject_prefix(g, g->proj_tmp, 0, nullptr, st));
-        CBCT_TRY(op_backproject_gather(g, g->proj_tmp, st));              // P^T (P f - Y)        a3
-        if (n_inner == 0) {
-            CBCT_TRY(op_combine(g, f, c, 1, g->vol_a, st));               // max(f - c G, 0)      a4+a6
-            CBCT_CUDA(cudaMemcpyAsync(f, g->vol_a, g->n_vox() * sizeof(float), cudaMemcpyDeviceToDevice, st));
+        if (g->bp_mode == CBCT_BACKPROJECTOR_EQ2) {
+            // the paper's step 1 (P:87 with eq. 2): dE2/df = (2/(N_theta A)) B r, so gv = f - c (dV/(du dv)) B r
+            const float c2 = (float)((double)c * (g->hx * g->hy * g->hz) / (g->du * g->dv));
+            CBCT_TRY(op_forward_padded(g, g->proj_tmp, d_Y, 2, st));      // P f - Y              a1+a2
+            if (n_inner == 0) {
+                CBCT_TRY(op_backproject_eq2(g, g->proj_tmp, f, c2, 1, g->vol_a, st));
+                CBCT_CUDA(cudaMemcpyAsync(f, g->vol_a, g->n_vox() * sizeof(float), cudaMemcpyDeviceToDevice, st));
+            } else {
+                CBCT_TRY(op_backproject_eq2(g, g->proj_tmp, f, c2, 0, g->vol_a, st));          // a3 (eq. 2) + a4
+                CBCT_TRY(tv_inner(g, g->vol_a, g->vol_a, f, beta, eps, omega, n_inner, 1, st));
+            }
         } else {
-            CBCT_TRY(op_combine(g, f, c, 0, g->vol_a, st));               // gv = f - c G         a4
-            CBCT_TRY(tv_inner(g, g->vol_a, g->vol_a, f, beta, eps, omega, n_inner, 1, st));   // u0 = gv (Q7); a5 + a6
+            CBCT_TRY(op_forward_padded(g, g->proj_tmp, d_Y, 1, st));          // l (P f - Y)          a1+a2
+            CBCT_TRY(op_backproject_prefix(g, g->proj_tmp, 0, nullptr, st));
+            CBCT_TRY(op_backproject_gather(g, g->proj_tmp, st));              // P^T (P f - Y)        a3
+            if (n_inner == 0) {
+                CBCT_TRY(op_combine(g, f, c, 1, g->vol_a, st));               // max(f - c G, 0)      a4+a6
+                CBCT_CUDA(cudaMemcpyAsync(f, g->vol_a, g->n_vox() * sizeof(float), cudaMemcpyDeviceToDevice, st));
+            } else {
+                CBCT_TRY(op_combine(g, f, c, 0, g->vol_a, st));               // gv = f - c G         a4
+                CBCT_TRY(tv_inner(g, g->vol_a, g->vol_a, f, beta, eps, omega, n_inner, 1, st));   // u0 = gv (Q7); a5 + a6
+            }
         }
         if (trace) {
             double e3[3];
@@ -163,7 +190,10 @@ extern "C" cbct_status cbct_fbs_reconstruct(const cbct_geometry *gc, const float
     // level handles, finest first
     std::vector<cbct_geometry *> lev(n_levels);
     lev[0] = mut(gc);
-    for (int l = 1; l < n_levels; ++l) CBCT_TRY(cbct_geometry_coarsen(lev[l - 1], &lev[l], nullptr));
+    for (int l = 1; l < n_levels; ++l) {
+        CBCT_TRY(cbct_geometry_coarsen(lev[l - 1], &lev[l], nullptr));
+        lev[l]->bp_mode = lev[0]->bp_mode;
+    }
 
     // data per level: level 0 uses d_Y, coarser levels their own binned copy
     std::vector<const float *> Y(n_levels);

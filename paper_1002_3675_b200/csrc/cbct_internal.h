@@ -84,6 +84,8 @@ struct cbct_geometry {
     float *host_stage_vol = nullptr, *host_stage_proj = nullptr, *host_stage_vol2 = nullptr;  // device staging for *_host
     unsigned long long bytes = 0;
 
+    int bp_mode = 0;                          // step 1 of A1: 0 exact transpose, 1 eq. 2 (cbct_set_backprojector)
+
     // multigrid
     cbct_geometry *coarse = nullptr;
     int coarsen_flags[4] = {0, 0, 0, 0};
@@ -145,7 +147,7 @@ inline size_t pad_elems(const cbct_geometry *g, int c)
 // ---- operators (device pointers, async on stream) ---------------------------------------------
 // projector.cu
 cbct_status op_pad_copies(cbct_geometry *g, const float *d_vol, cudaStream_t st);
-// mode 0: out = P f ; mode 1: out = l * (P f - Y)  (scaled residual for the gather)
+// mode 0: out = P f ; mode 1: out = l * (P f - Y)  (scaled residual for the gather) ; mode 2: out = P f - Y
 cbct_status op_forward_padded(cbct_geometry *g, float *d_out, const float *d_Y, int mode, cudaStream_t st);
 // backprojector.cu : gathers of the (already l-scaled) projections into G_cls[0], G_cls[1].
 // op_backproject_prefix builds the prefix sums along v that the gather reads (scale != 0: of l * d_in,
@@ -155,6 +157,9 @@ cbct_status op_backproject_gather(cbct_geometry *g, const float *d_scaled, cudaS
 // out = G1 + G0^T                         (f == nullptr)
 // out = f - c (G1 + G0^T), optionally clamped at 0   (f != nullptr)
 cbct_status op_combine(cbct_geometry *g, const float *f, float c, int clamp, float *out, cudaStream_t st);
+// backprojector_eq2.cu : out = B r (eq. 2, f == nullptr) or out = f - c (B r) [clamped]
+cbct_status op_backproject_eq2(cbct_geometry *g, const float *d_proj, const float *f, float c, int clamp, float *out,
+                               cudaStream_t st);
 // tv.cu
 cbct_status op_tv_sweep(cbct_geometry *g, const float *u_in, const float *gv, float *u_out,
                         float beta, float eps, float dt, int clamp, cudaStream_t st);

@@ -167,6 +167,7 @@ forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, c
             const size_t o = ((size_t)a * d.nv + v) * d.nu + u;
             float val = len * acc[q];
             if (mode == 1) val = len * (val - __ldg(Y + o));
+            else if (mode == 2) val -= __ldg(Y + o);
             out[o] = val;
         }
     }

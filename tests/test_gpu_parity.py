@@ -281,3 +281,51 @@ def test_host_entry_points(cuda_lib, dev):
     cb.tv_prox_host(G, vol, u, 40.0, 1e-3, 1.0, 3)
     assert rel(u, o.tv_prox(g, vol.astype(np.float64), vol.astype(np.float64), 40.0, 1e-3, 1.0, 3)) <= TOL_OP
     G.close()
+
+
+# ---- NEXT-1: the paper's eq. 2 backprojector ---------------------------------------------
+@pytest.mark.parametrize("name", ["c1", "aniso_ragged", "odd_dims_axis_angles", "wide_detector_misses"])
+def test_backproject_eq2_matches_oracle(cuda_lib, dev, name):
+    import torch
+    cb = cuda_lib
+    g = GEOMS[name]()
+    G = cb.Geometry.from_synth(g)
+    vol = f32(smooth_phantom(g, 3) if name != "c1" else make_config("c1").volume())
+    q = f32(o.forward(g, vol.astype(np.float64)))              # phantom-like projections
+    b = torch.empty(G.vol_shape, device=dev)
+    cb.backproject_eq2(G, to_dev(q, dev), b)
+    torch.cuda.synchronize()
+    assert rel(b.cpu().numpy(), o.backproject_eq2(g, q.astype(np.float64))) <= TOL_OP
+    # Gaussian images: every interpolation weight matters (fp32 position of (u*,v*) ~ 3e-5 pixel): stated bound 5e-5
+    y = f32(gaussian_field(g.proj_shape, 12))
+    cb.backproject_eq2(G, to_dev(y, dev), b)
+    torch.cuda.synchronize()
+    assert rel(b.cpu().numpy(), o.backproject_eq2(g, y.astype(np.float64))) <= 5e-5
+    G.close()
+
+
+def test_fbs_with_eq2_backprojector_matches_oracle(cuda_lib, dev):
+    """Algorithm A1 as the paper ran it (eq. 2 in step 1) on c1, 2 levels x 6 iterations, against the oracle."""
+    import torch
+    from oracle import fbs
+    cb = cuda_lib
+    cfg = make_config("c1")
+    g = cfg.geom
+    G = cb.Geometry.from_synth(g)
+    Y = f32(cfg.projections())
+    cb.set_backprojector(G, cb.BACKPROJECTOR_EQ2)
+    f = torch.empty(G.vol_shape, device=dev)
+    cb.fbs_reconstruct(G, to_dev(Y, dev), None, 2, [6, 6], cfg.n_inner, cfg.step, cfg.mu, cfg.eps, cfg.omega, f)
+    torch.cuda.synchronize()
+    ref = fbs.fbs_reconstruct(g, Y.astype(np.float64), None, 2, [6, 6], cfg.n_inner, cfg.step, cfg.mu, cfg.eps, cfg.omega,
+                              backprojector="eq2")
+    assert rel(f.cpu().numpy(), ref) <= TOL_RECON
+    # and the default is untouched by the option of another handle
+    G2 = cb.Geometry.from_synth(g)
+    f2 = torch.empty(G.vol_shape, device=dev)
+    cb.fbs_reconstruct(G2, to_dev(Y, dev), None, 1, [3], cfg.n_inner, cfg.step, cfg.mu, cfg.eps, cfg.omega, f2)
+    ref2 = fbs.fbs_reconstruct(g, Y.astype(np.float64), None, 1, [3], cfg.n_inner, cfg.step, cfg.mu, cfg.eps, cfg.omega)
+    assert rel(f2.cpu().numpy(), ref2) <= TOL_RECON
+    with pytest.raises(cb.CbctError):
+        cb.set_backprojector(G, 7)
+    G.close(); G2.close()
