@@ -271,6 +271,20 @@ def run_gpu(args):
              "ms_per_step_by_kernel": {k: v[0] / K for k, v in prof.items()}}
     if not args.no_recon and world == 1:
         extra["sec_per_fbs_recon_c3"] = time_c3_recon(cb, dev, st)
+        # NEXT-1 (not part of `value`): the paper's eq. 2 backprojector, alone at c2 and inside the c3 reconstruction
+        extra["sec_per_fbs_recon_c3_eq2"] = time_c3_recon(cb, dev, st, eq2=True)
+        q = torch.empty(g.proj_shape, device=dev)
+        b = torch.empty(g.vol_shape, device=dev)
+        ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(st):
+            cb.forward(G, d_f, q, stream=st)
+            cb.backproject_eq2(G, q, b, stream=st)
+            ea.record(st)
+            for _ in range(5):
+                cb.backproject_eq2(G, q, b, stream=st)
+            eb.record(st)
+        torch.cuda.synchronize()
+        extra["gups_backproject_eq2"] = g.n_vox * g.n_angles / (ea.elapsed_time(eb) / 5e3) / 1e9
     cpu = cpu_baseline_sample(cfg, n_angles=args.cpu_angles) if world == 1 and not args.no_cpu else None
 
     line = {
@@ -295,7 +309,7 @@ def run_gpu(args):
         dist.destroy_process_group()
 
 
-def time_c3_recon(cb, dev, st):
+def time_c3_recon(cb, dev, st, eq2=False):
     """seconds per full c3 reconstruction (2 levels x 100 outer x 10 inner; noisy 40-view data)."""
     import torch
     from cbct_synth import make_config
@@ -303,6 +317,8 @@ def time_c3_recon(cb, dev, st):
     g = cfg.geom
     Y = torch.from_numpy(np.ascontiguousarray(cfg.projections(), dtype=np.float32)).to(dev)
     G = cb.Geometry.from_synth(g)
+    if eq2:
+        cb.set_backprojector(G, cb.BACKPROJECTOR_EQ2)
     f = torch.empty(g.vol_shape, device=dev)
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with torch.cuda.stream(st):

@@ -42,15 +42,21 @@ def energy(g, f, Y, mu: float, eps: float, Pf: Optional[np.ndarray] = None) -> d
 # ----------------------------------------------------------------------------------------
 def fbs_level(g, Y, f0, n_outer: int, n_inner: int, step: float, mu: float, eps: float,
               omega: float = 1.0, u0_mode: str = "g", clamp: bool = True,
-              trace: Optional[list] = None, backprojector: str = "exact") -> np.ndarray:
-    """backprojector = "exact": dE2/df through the matrix transpose (P:95, the hot path);
+              trace: Optional[list] = None, backprojector: str = "exact",
+              rel_tol: float = 0.0, iters_done: Optional[list] = None) -> np.ndarray:
+    """rel_tol > 0: "Repeat ... until convergence" read as: stop after the first iteration whose update
+    satisfies ||f_new - f_old||_2 <= rel_tol ||f_new||_2 (NEXT-2; n_outer is then the maximum count);
+    the number of iterations run is appended to iters_done.
+    backprojector = "exact": dE2/df through the matrix transpose (P:95, the hot path);
     "eq2": through the paper's eq. 2: dE2/df(x) = (2/(N_theta A)) (B r)(x), so step 1 reads
     g = f - (mu V/beta) dE2/df = f - c (dV/(du dv)) (B r) with the same c."""
     o = _prims()
     f = np.array(f0, dtype=np.float64, copy=True)
     beta = mu / step
     c = 2.0 * step * g.n_vox / (g.n_angles * g.n_pix)
+    done = 0
     for _ in range(n_outer):
+        f_old = f
         r = o.forward(g, f) - Y                      # P f - Y            (P:99)
         if backprojector == "exact":
             G = o.backproject(g, r)                  # P^T (P f - Y)      (P:95)
@@ -62,6 +68,11 @@ def fbs_level(g, Y, f0, n_outer: int, n_inner: int, step: float, mu: float, eps:
         f = np.maximum(u, 0.0) if clamp else u       # step 3             (Q18)
         if trace is not None:
             trace.append(energy(g, f, Y, mu, eps))
+        done += 1
+        if rel_tol > 0.0 and np.sqrt(np.sum((f - f_old) ** 2)) <= rel_tol * np.sqrt(np.sum(f ** 2)):
+            break
+    if iters_done is not None:
+        iters_done.append(done)
     return f
 
 
@@ -150,7 +161,8 @@ def prolong(c: np.ndarray, axes) -> np.ndarray:
 
 def fbs_reconstruct(g, Y, f0, n_levels: int, n_outer: Sequence[int], n_inner: int, step: float,
                     mu: float, eps: float, omega: float = 1.0, u0_mode: str = "g",
-                    clamp: bool = True, trace: Optional[list] = None, backprojector: str = "exact") -> np.ndarray:
+                    clamp: bool = True, trace: Optional[list] = None, backprojector: str = "exact",
+                    rel_tol: float = 0.0, iters_done: Optional[list] = None) -> np.ndarray:
     """O6: run O5 at the coarsest level from f0 (zeros if None; a caller's fine-grid f0 is
     restricted down), prolong to the next level, repeat; n_outer is listed coarsest first.
     n_levels = 1 is exactly O5."""
@@ -167,7 +179,8 @@ def fbs_reconstruct(g, Y, f0, n_levels: int, n_outer: Sequence[int], n_inner: in
             f = restrict_volume(f, ax)
     for n, lev in enumerate(range(n_levels - 1, -1, -1)):
         f = fbs_level(geoms[lev], Ys[lev], f, n_outer[n], n_inner, step, mu, eps, omega,
-                      u0_mode=u0_mode, clamp=clamp, trace=trace, backprojector=backprojector)
+                      u0_mode=u0_mode, clamp=clamp, trace=trace, backprojector=backprojector,
+                      rel_tol=rel_tol, iters_done=iters_done)
         if lev > 0:
             f = prolong(f, axes[lev - 1])
     return f

@@ -4,6 +4,7 @@ import pytest
 from scipy.optimize import nnls
 
 import oracle as o
+from oracle import fbs
 from cbct_synth import Geometry, make_config
 from cbct_synth.geometry import equispaced_angles
 
@@ -165,3 +166,27 @@ def test_I13_c1_quality_sanity():
     assert errs[-1] < 0.6 * errs[0]
     E = np.array([t["E_eps"] for t in tr])
     assert np.all(np.diff(E) < 0)
+
+
+def test_stopping_rule_is_the_first_iteration_below_the_tolerance():
+    """NEXT-2 ("Repeat ... until convergence"): with rel_tol the loop stops after the first iteration
+    whose relative update is <= rel_tol; the count is checked against fixed-count runs, rel_tol = 0 is the
+    fixed-count loop, a huge rel_tol stops after one iteration."""
+    cfg = make_config("c1", shrink=2)
+    g, Y = cfg.geom, cfg.projections()
+    args = (cfg.n_inner, cfg.step, cfg.mu, cfg.eps, cfg.omega)
+    traj = [np.zeros(g.vol_shape)]
+    for n in range(1, 13):
+        traj.append(fbs.fbs_reconstruct(g, Y, None, 1, [n], *args))
+    change = [np.linalg.norm(traj[n] - traj[n - 1]) / np.linalg.norm(traj[n]) for n in range(1, 13)]
+    assert all(b < a for a, b in zip(change[2:], change[3:]))          # the update shrinks on this problem
+    tol = 0.5 * (change[6] + change[7])                                # clear margin: stops at iteration 8
+    done = []
+    f = fbs.fbs_reconstruct(g, Y, None, 1, [12], *args, rel_tol=tol, iters_done=done)
+    first = next(n for n in range(1, 13) if change[n - 1] <= tol)
+    assert done == [first] and first == 8
+    assert np.array_equal(f, traj[first])
+    done = []
+    assert np.array_equal(fbs.fbs_reconstruct(g, Y, None, 1, [5], *args, rel_tol=0.0, iters_done=done), traj[5]) and done == [5]
+    done = []
+    assert np.array_equal(fbs.fbs_reconstruct(g, Y, None, 1, [5], *args, rel_tol=1e9, iters_done=done), traj[1]) and done == [1]
