@@ -172,6 +172,19 @@ cbct_status cbct_fbs_reconstruct(const cbct_geometry *g, const float *d_Y, const
                                  float *d_f_out, double *h_energy_trace, void *cuda_stream);
 
 /*
+ * NEXT-2. The same cascade with the paper's "Repeat ... until convergence" read as a stopping rule:
+ * a level stops after the first outer iteration whose update satisfies
+ *   || f_new - f_old ||_2 <= rel_tol || f_new ||_2        (sums accumulated in fp64 on the device),
+ * or after n_outer_max_per_level[] iterations (COARSEST FIRST).  rel_tol == 0 is cbct_fbs_reconstruct.
+ * h_iters_per_level: NULL, or n_levels ints receiving the iterations run per level (coarsest first).
+ * Synchronises the stream once per outer iteration when rel_tol > 0.
+ */
+cbct_status cbct_fbs_reconstruct_until(const cbct_geometry *g, const float *d_Y, const float *d_f0,
+                                       int n_levels, const int *n_outer_max_per_level, int n_tv_inner,
+                                       float step, float mu, float eps, float omega, float rel_tol,
+                                       float *d_f_out, int *h_iters_per_level, void *cuda_stream);
+
+/*
  * Host-buffer variants (end-to-end path): same operations with HOST pointers; each call copies its
  * inputs host->device and its result device->host on `cuda_stream` (use pinned host memory for
  * full copy speed) and returns after synchronising the stream.

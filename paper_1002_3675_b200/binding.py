@@ -16,7 +16,7 @@ STATUS = {0: "CBCT_OK", 1: "CBCT_ERR_INVALID_ARG", 2: "CBCT_ERR_SHAPE", 3: "CBCT
 SYMBOLS = (
     "cbct_geometry_create", "cbct_geometry_destroy", "cbct_geometry_query", "cbct_geometry_coarsen",
     "cbct_forward", "cbct_backproject", "cbct_backproject_eq2", "cbct_set_backprojector", "cbct_tv_prox", "cbct_prolong", "cbct_restrict", "cbct_bin2x2",
-    "cbct_energy", "cbct_fbs_reconstruct", "cbct_forward_host", "cbct_backproject_host", "cbct_tv_prox_host",
+    "cbct_energy", "cbct_fbs_reconstruct", "cbct_fbs_reconstruct_until", "cbct_forward_host", "cbct_backproject_host", "cbct_tv_prox_host",
     "cbct_fbs_reconstruct_host", "cbct_profile_enable", "cbct_profile_read", "cbct_launch_count", "cbct_device_bytes", "cbct_last_error",
 )
 
@@ -57,6 +57,7 @@ def load():
     L.cbct_bin2x2.argtypes = [vp, fp, fp, vp]
     L.cbct_energy.argtypes = [vp, fp, fp, f, f, dp, vp]
     L.cbct_fbs_reconstruct.argtypes = [vp, fp, fp, i, ip, i, f, f, f, f, fp, dp, vp]
+    L.cbct_fbs_reconstruct_until.argtypes = [vp, fp, fp, i, ip, i, f, f, f, f, f, fp, ip, vp]
     L.cbct_forward_host.argtypes = [vp, fp, fp, vp]
     L.cbct_backproject_host.argtypes = [vp, fp, fp, vp]
     L.cbct_tv_prox_host.argtypes = [vp, fp, fp, f, f, f, i, vp]
@@ -256,6 +257,20 @@ def fbs_reconstruct(g: Geometry, d_Y, d_f0, n_levels, n_outer, n_inner, step, mu
                                        int(n_levels), arr, int(n_inner), float(step), float(mu), float(eps),
                                        float(omega), _dev(d_f_out, g.n_vox, "d_f_out"), tr, _stream(stream)))
     return list(tr)[:total] if trace else None
+
+
+def fbs_reconstruct_until(g: Geometry, d_Y, d_f0, n_levels, n_outer_max, n_inner, step, mu, eps, omega, rel_tol, d_f_out,
+                          stream=None):
+    """The cascade with the stopping rule ||f_new - f_old|| <= rel_tol ||f_new|| per level; returns the
+    iterations run per level (coarsest first)."""
+    arr, _ = _outer(n_levels, n_outer_max)
+    iters = (C.c_int * int(n_levels))()
+    _check(load().cbct_fbs_reconstruct_until(g._h, _dev(d_Y, g.n_proj, "d_Y"),
+                                             None if d_f0 is None else _dev(d_f0, g.n_vox, "d_f0"),
+                                             int(n_levels), arr, int(n_inner), float(step), float(mu), float(eps),
+                                             float(omega), float(rel_tol), _dev(d_f_out, g.n_vox, "d_f_out"), iters,
+                                             _stream(stream)))
+    return list(iters)
 
 
 def forward_host(g: Geometry, h_vol, h_proj, stream=None):

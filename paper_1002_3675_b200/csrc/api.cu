@@ -136,14 +136,23 @@ extern "C" cbct_status cbct_energy(const cbct_geometry *gc, const float *d_f, co
 }
 
 // One level of Algorithm A1: f (in/out, level-sized device buffer).
+// rel_tol > 0: stop after the first iteration with ||f_new - f_old||_2 <= rel_tol ||f_new||_2 (NEXT-2; sums in fp64,
+// one stream synchronise per iteration); *iters receives the number of iterations run.
 static cbct_status fbs_level(cbct_geometry *g, const float *d_Y, float *f, int n_outer, int n_inner, float step,
-                             float mu, float eps, float omega, double *trace, cudaStream_t st)
+                             float mu, float eps, float omega, double *trace, float rel_tol, int *iters, cudaStream_t st)
 {
+    if (rel_tol > 0.f) {
+        CBCT_TRY(ensure(g, &g->vol_c, g->n_vox()));
+        CBCT_TRY(ensure(g, &g->red_out, (size_t)2));
+        if (!g->h_red) CBCT_CUDA(cudaMallocHost((void **)&g->h_red, 2 * sizeof(double)));
+    }
+    if (iters) *iters = 0;
     CBCT_TRY(ensure(g, &g->proj_tmp, g->n_proj(), true));
     CBCT_TRY(ensure(g, &g->vol_a, g->n_vox()));
     const float beta = mu / step;
     const float c = (float)(2.0 * (double)step * (double)g->n_vox() / ((double)g->na * g->nu * g->nv));
     for (int it = 0; it < n_outer; ++it) {
+        if (rel_tol > 0.f) CBCT_CUDA(cudaMemcpyAsync(g->vol_c, f, g->n_vox() * sizeof(float), cudaMemcpyDeviceToDevice, st));
         CBCT_TRY(op_pad_copies(g, f, st));
         if (g->bp_mode == CBCT_BACKPROJECTOR_EQ2) {
             // the paper's step 1 (P:87 with eq. 2): dE2/df = (2/(N_theta A)) B r, so gv = f - c (dV/(du dv)) B r
@@ -173,13 +182,21 @@ static cbct_status fbs_level(cbct_geometry *g, const float *d_Y, float *f, int n
             CBCT_TRY(energy_impl(g, f, d_Y, mu, eps, e3, st));
             trace[it] = e3[0];
         }
+        if (iters) *iters = it + 1;
+        if (rel_tol > 0.f) {
+            CBCT_TRY(op_sumsq_diff(g, f, g->vol_c, g->n_vox(), g->red_out + 0, st));
+            CBCT_TRY(op_sumsq_diff(g, f, nullptr, g->n_vox(), g->red_out + 1, st));
+            CBCT_CUDA(cudaMemcpyAsync(g->h_red, g->red_out, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+            CBCT_CUDA(cudaStreamSynchronize(st));
+            if (std::sqrt(g->h_red[0]) <= (double)rel_tol * std::sqrt(g->h_red[1])) break;
+        }
     }
     return CBCT_OK;
 }
 
-extern "C" cbct_status cbct_fbs_reconstruct(const cbct_geometry *gc, const float *d_Y, const float *d_f0, int n_levels,
-                                            const int *n_outer, int n_inner, float step, float mu, float eps,
-                                            float omega, float *d_f_out, double *trace, void *stream)
+static cbct_status fbs_cascade(const cbct_geometry *gc, const float *d_Y, const float *d_f0, int n_levels,
+                               const int *n_outer, int n_inner, float step, float mu, float eps, float omega,
+                               float *d_f_out, double *trace, float rel_tol, int *iters_per_level, void *stream)
 {
     REQUIRE(gc && d_Y && d_f_out && n_outer, "cbct_fbs_reconstruct: NULL argument");
     REQUIRE(n_levels >= 1 && n_levels <= 16 && n_inner >= 0, "cbct_fbs_reconstruct: n_levels < 1 (or > 16) or n_tv_inner < 0");
@@ -222,11 +239,29 @@ extern "C" cbct_status cbct_fbs_reconstruct(const cbct_geometry *gc, const float
     int done = 0;
     for (int l = L; l >= 0; --l) {
         const int n = n_outer[L - l];
-        CBCT_TRY(fbs_level(lev[l], Y[l], F[l], n, n_inner, step, mu, eps, omega, trace ? trace + done : nullptr, st));
+        CBCT_TRY(fbs_level(lev[l], Y[l], F[l], n, n_inner, step, mu, eps, omega, trace ? trace + done : nullptr, rel_tol,
+                           iters_per_level ? iters_per_level + (L - l) : nullptr, st));
         done += n;
         if (l > 0) CBCT_TRY(op_prolong(lev[l - 1], F[l], F[l - 1], st));
     }
     return CBCT_OK;
+}
+
+extern "C" cbct_status cbct_fbs_reconstruct(const cbct_geometry *gc, const float *d_Y, const float *d_f0, int n_levels,
+                                            const int *n_outer, int n_inner, float step, float mu, float eps,
+                                            float omega, float *d_f_out, double *trace, void *stream)
+{
+    return fbs_cascade(gc, d_Y, d_f0, n_levels, n_outer, n_inner, step, mu, eps, omega, d_f_out, trace, 0.f, nullptr, stream);
+}
+
+extern "C" cbct_status cbct_fbs_reconstruct_until(const cbct_geometry *gc, const float *d_Y, const float *d_f0, int n_levels,
+                                                  const int *n_outer_max, int n_inner, float step, float mu, float eps,
+                                                  float omega, float rel_tol, float *d_f_out, int *h_iters_per_level,
+                                                  void *stream)
+{
+    REQUIRE(rel_tol >= 0.f, "cbct_fbs_reconstruct_until: rel_tol < 0");
+    return fbs_cascade(gc, d_Y, d_f0, n_levels, n_outer_max, n_inner, step, mu, eps, omega, d_f_out, nullptr, rel_tol,
+                       h_iters_per_level, stream);
 }
 
 // ---- host-buffer variants ----------------------------------------------------------------------

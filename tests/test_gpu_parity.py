@@ -329,3 +329,37 @@ def test_fbs_with_eq2_backprojector_matches_oracle(cuda_lib, dev):
     with pytest.raises(cb.CbctError):
         cb.set_backprojector(G, 7)
     G.close(); G2.close()
+
+
+def test_fbs_until_stops_where_the_oracle_stops(cuda_lib, dev):
+    """NEXT-2: the stopping rule ||f_new - f_old|| <= rel_tol ||f_new|| ("until convergence").  The tolerance
+    sits half-way between two consecutive relative updates of the oracle's trajectory, so the fp32 path and the
+    fp64 oracle take the same decision; iteration counts and volumes must then match."""
+    import torch
+    from oracle import fbs
+    cb = cuda_lib
+    cfg = make_config("c1")
+    g = cfg.geom
+    G = cb.Geometry.from_synth(g)
+    Y = f32(cfg.projections())
+    args = (cfg.n_inner, cfg.step, cfg.mu, cfg.eps, cfg.omega)
+    Y64 = Y.astype(np.float64)
+    prev, change = np.zeros(g.vol_shape), []
+    for n in range(1, 9):
+        cur = fbs.fbs_reconstruct(g, Y64, None, 1, [n], *args)
+        change.append(np.linalg.norm(cur - prev) / np.linalg.norm(cur))
+        prev = cur
+    tol = 0.5 * (change[4] + change[5])
+    done = []
+    ref = fbs.fbs_reconstruct(g, Y64, None, 1, [8], *args, rel_tol=tol, iters_done=done)
+    f = torch.empty(G.vol_shape, device=dev)
+    iters = cb.fbs_reconstruct_until(G, to_dev(Y, dev), None, 1, [8], *args, tol, f)
+    assert iters == done and 1 < iters[0] < 8
+    assert rel(f.cpu().numpy(), ref) <= TOL_RECON
+    # rel_tol = 0 is the fixed-count loop; a huge tolerance stops every level after one iteration
+    iters = cb.fbs_reconstruct_until(G, to_dev(Y, dev), None, 2, [3, 2], *args, 0.0, f)
+    assert iters == [3, 2]
+    ref2 = fbs.fbs_reconstruct(g, Y64, None, 2, [3, 2], *args)
+    assert rel(f.cpu().numpy(), ref2) <= TOL_RECON
+    assert cb.fbs_reconstruct_until(G, to_dev(Y, dev), None, 2, [3, 2], *args, 1e9, f) == [1, 1]
+    G.close()
