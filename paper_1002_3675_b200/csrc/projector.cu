@@ -101,7 +101,7 @@ forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, c
         const float dirpos = r.sm >= 0.f ? 1.f : 0.f;
         const int dneg = r.sm >= 0.f ? 0 : 1;
         float zeta[V], inv_sz[V], zbnd[V];
-        int rowoff[V];                                          // element offsets fit 32 bits (checked at geometry creation)
+        int krow[V], rowoff[V];                                          // element offsets fit 32 bits (checked at geometry creation)
         const int pstride = (int)cg.plane_stride;
         const float e0 = (float)(lo_w - cg.ioff);
         const float T0 = fmaf(e0, r.dt, r.tc);
@@ -113,8 +113,8 @@ forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, c
             const float Za = fmaf(T0, zeta[q], d.zfrac);
             const float kf = floorf(Za);
             zbnd[q] = kf + (inv_sz[q] >= 0.f ? 1.f : 0.f);
-            const int k = (int)kf + d.koff;
-            rowoff[q] = (min(max(k, -kPadK), d.nz + kPadK - 1) + kPadK) * pstride;
+            krow[q] = (int)kf + d.koff;
+            rowoff[q] = (min(max(krow[q], -kPadK), d.nz + kPadK - 1) + kPadK) * pstride;
         }
         const float *base = vol + kPadLo;
         for (int i = lo_w; i < hi_w; ++i) {
@@ -144,9 +144,10 @@ forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, c
 #pragma unroll
             for (int q = 0; q < V; ++q) {
                 if (b[q] < 1.f) {
-                    const float zs = inv_sz[q] >= 0.f ? 1.f : -1.f;
-                    const int k1 = (int)(zbnd[q] - (zs > 0.f ? 1.f : 0.f) + zs) + d.koff;
-                    const int rowoff1 = (min(max(k1, -kPadK), d.nz + kPadK - 1) + kPadK) * pstride;
+                    const bool upz = inv_sz[q] >= 0.f;
+                    const float zs = upz ? 1.f : -1.f;
+                    krow[q] += upz ? 1 : -1;                   // true z row (rows outside the pad read the outermost zero plane)
+                    const int rowoff1 = (min(max(krow[q], -kPadK), d.nz + kPadK - 1) + kPadK) * pstride;
                     const float *p = base + (rowoff[q] + off_i), *p1 = base + (rowoff1 + off_i);
                     const float c_r0 = a_ - fminf(a_, b[q]), c_r1 = 1.f - fmaxf(a_, b[q]);
                     const float c_lo = dneg ? c_r1 : c_r0, c_hi = dneg ? c_r0 : c_r1;
