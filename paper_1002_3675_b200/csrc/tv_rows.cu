@@ -87,9 +87,10 @@ tv_rows_kernel(const float *__restrict__ u_in, const float *__restrict__ gv, flo
     const size_t sxy = (size_t)nx * ny;
     const size_t rowoff = (size_t)max(y, 0) * nx;
 
-    float uc[XPT], un[XPT], qzp[XPT];
+    float uc[XPT], un[XPT], u2[XPT], qzp[XPT];
     const int zs = max(zc0 - 1, 0);
     load_row<XPT, VEC>(uc, u_in + (size_t)zs * sxy + rowoff, x0, nx, row_ok);
+    load_row<XPT, VEC>(un, u_in + (size_t)min(zs + 1, nz - 1) * sxy + rowoff, x0, nx, row_ok && zs + 1 < nz);
 #pragma unroll
     for (int e = 0; e < XPT; ++e) qzp[e] = 0.f;
     put_row<XPT>(B + ((zs & 1) * NW + w) * W, lane, uc);
@@ -98,7 +99,9 @@ tv_rows_kernel(const float *__restrict__ u_in, const float *__restrict__ gv, flo
     for (int z = zs; z < zc1; ++z) {
         const int cur = z & 1, nxt = cur ^ 1;
         const bool has_zp = z + 1 < nz;
-        load_row<XPT, VEC>(un, u_in + (size_t)min(z + 1, nz - 1) * sxy + rowoff, x0, nx, row_ok && has_zp);
+        // plane z+2 is requested now and consumed at the end of this iteration: its latency hides behind the
+        // fluxes and the barrier of plane z
+        load_row<XPT, VEC>(u2, u_in + (size_t)min(z + 2, nz - 1) * sxy + rowoff, x0, nx, row_ok && z + 2 < nz && z + 1 < zc1);
         put_row<XPT>(B + (nxt * NW + w) * W, lane, un);
         float g[XPT];
         const bool upd = do_upd && z >= zc0;
@@ -156,7 +159,7 @@ tv_rows_kernel(const float *__restrict__ u_in, const float *__restrict__ gv, flo
             }
         }
 #pragma unroll
-        for (int e = 0; e < XPT; ++e) { qzp[e] = qz[e]; uc[e] = un[e]; }
+        for (int e = 0; e < XPT; ++e) { qzp[e] = qz[e]; uc[e] = un[e]; un[e] = u2[e]; }
     }
 }
 
