@@ -10,6 +10,7 @@
 // buffered: one barrier per plane).  The first warp only produces qy for the row below it, the last
 // only publishes u for the row above it; the NW-2 rows in between are updated and stored.
 // HBM traffic per voxel and step: read u, read g, write u' (12 B), each once, as 16-byte accesses.
+
 #include "cbct_internal.h"
 
 namespace {
@@ -167,27 +168,37 @@ template <int XPT, bool VEC>
 cbct_status launch_rows(cbct_geometry *g, const float *u_in, const float *gv, float *u_out, float beta, float eps,
                         float dt, int clamp, cudaStream_t st)
 {
-    // warps per CTA: measured best on B200 (c2, nx = 256: 8; c3, nx = 512: 12 -- more rows amortise the two halo
-    // warps, fewer leave room for more CTAs per SM)
+    // warps per CTA: measured on B200 (more rows amortise the two halo warps, fewer leave room for more CTAs per SM)
 #ifndef CBCT_TV_NW
-    constexpr int NW = XPT >= 16 ? 12 : 8;
+    constexpr int NW = XPT >= 16 ? 6 : 10;
 #else
     constexpr int NW = CBCT_TV_NW;
-#endif
-#ifndef CBCT_TV_ZC
-#define CBCT_TV_ZC 16
 #endif
     constexpr int ROWS = NW - 2;
     auto kern = tv_rows_kernel<XPT, NW, VEC>;
     const size_t smem = (size_t)4 * NW * 32 * XPT * sizeof(float);
-    static bool attr_set = false;                 // per instantiation
-    if (!attr_set) {
+    static int slots = 0;                         // CTAs the device holds at once (per instantiation)
+    if (!slots) {
         CBCT_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
+        int dev = 0, sms = 0, per_sm = 0;
+        CBCT_CUDA(cudaGetDevice(&dev));
+        CBCT_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        CBCT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 32 * NW, smem));
+        slots = sms * (per_sm > 0 ? per_sm : 1);
     }
+    // z planes per CTA: a chunk of zc planes costs zc + 1 plane iterations (it recomputes the fluxes of the plane
+    // below it) and the grid runs in ceil(CTAs / slots) waves: take the chunk that minimises waves x (zc + 1)
     const int ytiles = (g->ny + ROWS - 1) / ROWS;
-    int zchunk = CBCT_TV_ZC;
-    if (ytiles * ((g->nz + zchunk - 1) / zchunk) < 296) zchunk /= 2;    // at least two CTAs per SM where the volume allows it
+    int zchunk = 8;
+    long best = -1;
+    for (int zc = 4; zc <= 64; ++zc) {
+        const long ctas = (long)ytiles * ((g->nz + zc - 1) / zc);
+        const long cost = ((ctas + slots - 1) / slots) * (zc + 1);
+        if (best < 0 || cost < best) { best = cost; zchunk = zc; }
+    }
+#ifdef CBCT_TV_ZC_FORCE
+    zchunk = CBCT_TV_ZC_FORCE;
+#endif
     dim3 grid(ytiles, (g->nz + zchunk - 1) / zchunk);
     const double hx = g->hx, hy = g->hy, hz = g->hz;
     kern<<<grid, 32 * NW, smem, st>>>(u_in, gv, u_out, g->nx, g->ny, g->nz, (float)(1.0 / (hx * hx)), (float)(1.0 / (hy * hy)),
