@@ -363,3 +363,28 @@ def test_fbs_until_stops_where_the_oracle_stops(cuda_lib, dev):
     assert rel(f.cpu().numpy(), ref2) <= TOL_RECON
     assert cb.fbs_reconstruct_until(G, to_dev(Y, dev), None, 2, [3, 2], *args, 1e9, f) == [1, 1]
     G.close()
+
+
+def test_short_scan_subset_reconstruction_matches_oracle(cuda_lib, dev):
+    """The shape of the paper's CatPhan experiment (379 views over 200 degrees, a subset of 40 used), shrunk:
+    every 9th-10th of 379 angles over 200 degrees, noisy data, 2-level cascade, against the oracle."""
+    import torch
+    from oracle import fbs
+    from cbct_synth import line_integrals, random_ellipsoids, poisson_log
+    cb = cuda_lib
+    all_angles = np.deg2rad(np.linspace(0.0, 200.0, 379, endpoint=False))
+    angles = all_angles[np.linspace(0, 378, 40).round().astype(int)]
+    g = Geometry(1000., 1500., angles, 64, 48, 3.0, 3.0, 32, 32, 16, 3.0, 3.0, 5.0)
+    rng = np.random.default_rng(600)
+    ells = random_ellipsoids(rng, 8, (g.nx * g.hx, g.ny * g.hy, g.nz * g.hz), (6.0, 25.0))
+    Y = f32(poisson_log(line_integrals(ells, g), 1e5, rng))
+    cfg = make_config("c1")
+    step = 0.5 * (g.nu * g.nv * g.du * g.dv) / (g.n_vox * g.hx * g.hy * g.hz * 140.0 * 1.6 ** 2)
+    mu = step * 4.0 * (2 / 3.0 ** 2 + 1 / 5.0 ** 2) / cfg.eps
+    G = cb.Geometry.from_synth(g)
+    f = torch.empty(G.vol_shape, device=dev)
+    cb.fbs_reconstruct(G, to_dev(Y, dev), None, 2, [8, 8], 5, step, mu, cfg.eps, 1.0, f)
+    torch.cuda.synchronize()
+    ref = fbs.fbs_reconstruct(g, Y.astype(np.float64), None, 2, [8, 8], 5, step, mu, cfg.eps, 1.0)
+    assert np.linalg.norm(ref) > 0 and rel(f.cpu().numpy(), ref) <= TOL_RECON
+    G.close()
