@@ -309,6 +309,64 @@ def run_gpu(args):
         dist.destroy_process_group()
 
 
+def run_sharded(args):
+    """--shard-angles (NEXT-4, not the default): ONE reconstruction step of c2 with the 40 views partitioned over
+    the ranks and one NCCL all-reduce of the gradient volume per outer iteration; strong scaling."""
+    import torch
+    import paper_1002_3675_b200 as cb
+    from paper_1002_3675_b200.sharded import CudaOps, fbs_reconstruct_sharded, shard_angles
+    from cbct_synth import make_config
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    cb.load()
+    cfg = make_config("c2")
+    g = cfg.geom
+    mine = shard_angles(g.n_angles, rank, world)
+    G = cb.Geometry.from_synth(g.with_angles(g.angles[mine]))
+    d_Y = torch.from_numpy(np.ascontiguousarray(cfg.projections(mine), dtype=np.float32)).to(dev)
+    ops = CudaOps(G, LEVELS)
+    state = {"f": torch.zeros(g.vol_shape, device=dev)}
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def step():
+        state["f"] = fbs_reconstruct_sharded(ops, d_Y, state["f"], LEVELS, [1] * LEVELS, N_INNER, cfg.step, cfg.mu, cfg.eps,
+                                             cfg.omega, g.n_angles, dist)
+
+    for _ in range(args.warmup):
+        step()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    with ClockSampler(local) as clk:
+        for a, b in ev:
+            flush.fill_(1)
+            a.record()
+            step()
+            b.record()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+    t = max_over_ranks(sum(a.elapsed_time(b) for a, b in ev) / 1e3, dist, dev)
+    if rank == 0:
+        updates = 2.0 * sum(nvox * g.n_angles for nvox, _ in level_dims(g, LEVELS))
+        print(json.dumps({"metric": METRIC, "value": whole_job_value(1, updates, args.steps, t), "unit": UNIT, "n_gpus": world,
+                          "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps,
+                          "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                          "config": {"workload": "c2, one reconstruction step with its 40 views sharded over the ranks",
+                                     "parallelism": f"angles sharded over {world} rank(s), one all-reduce of the gradient "
+                                                    "volume per outer iteration (NEXT-4)", "l2": "flushed between steps"},
+                          "clocks": clk.summary()}))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def time_c3_recon(cb, dev, st, eq2=False):
     """seconds per full c3 reconstruction (2 levels x 100 outer x 10 inner; noisy 40-view data)."""
     import torch
@@ -390,10 +448,14 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
     ap.add_argument("--no-recon", action="store_true", help="skip the full c3 reconstruction timing")
     ap.add_argument("--cpu-angles", type=int, default=8)
+    ap.add_argument("--shard-angles", action="store_true",
+                    help="NEXT-4: shard the views of ONE reconstruction over the ranks (strong scaling) instead of replicas")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
     if args.impl == "reference":
         run_reference(args)
+    elif args.shard_angles:
+        run_sharded(args)
     else:
         run_gpu(args)
 

@@ -185,6 +185,21 @@ cbct_status cbct_fbs_reconstruct_until(const cbct_geometry *g, const float *d_Y,
                                        float *d_f_out, int *h_iters_per_level, void *cuda_stream);
 
 /*
+ * NEXT-4. The two halves of one outer iteration of A1, for drivers that put an exchange step between them: with
+ * the angle list partitioned over several GPUs (one handle per GPU holding its share of the angles and of d_Y),
+ * every GPU computes its partial data gradient, the partial volumes are summed (one all-reduce), and every GPU
+ * applies the same prox step.  P^T over a subset of the angles is an exact partial sum of the full P^T.
+ *   cbct_data_gradient : d_G = P^T (P d_f - d_Y) over this handle's angles (with CBCT_BACKPROJECTOR_EQ2:
+ *                        (dV/(du dv)) B (P d_f - d_Y)).  d_G is overwritten; must not alias d_f.
+ *   cbct_prox_step     : d_f_out = max(0, TVprox(d_f - c d_G)), n_inner steps with beta, eps, omega as in
+ *                        cbct_tv_prox; c = 2 step N_vox / (N_theta N_pix) with the TOTAL number of angles.
+ *                        d_f_out may alias d_f, not d_G.
+ */
+cbct_status cbct_data_gradient(const cbct_geometry *g, const float *d_f, const float *d_Y, float *d_G, void *cuda_stream);
+cbct_status cbct_prox_step(const cbct_geometry *g, const float *d_f, const float *d_G, float c, float beta,
+                           float eps, float omega, int n_inner, float *d_f_out, void *cuda_stream);
+
+/*
  * Host-buffer variants (end-to-end path): same operations with HOST pointers; each call copies its
  * inputs host->device and its result device->host on `cuda_stream` (use pinned host memory for
  * full copy speed) and returns after synchronising the stream.

@@ -16,7 +16,7 @@ STATUS = {0: "CBCT_OK", 1: "CBCT_ERR_INVALID_ARG", 2: "CBCT_ERR_SHAPE", 3: "CBCT
 SYMBOLS = (
     "cbct_geometry_create", "cbct_geometry_destroy", "cbct_geometry_query", "cbct_geometry_coarsen",
     "cbct_forward", "cbct_backproject", "cbct_backproject_eq2", "cbct_set_backprojector", "cbct_tv_prox", "cbct_prolong", "cbct_restrict", "cbct_bin2x2",
-    "cbct_energy", "cbct_fbs_reconstruct", "cbct_fbs_reconstruct_until", "cbct_forward_host", "cbct_backproject_host", "cbct_tv_prox_host",
+    "cbct_energy", "cbct_data_gradient", "cbct_prox_step", "cbct_fbs_reconstruct", "cbct_fbs_reconstruct_until", "cbct_forward_host", "cbct_backproject_host", "cbct_tv_prox_host",
     "cbct_fbs_reconstruct_host", "cbct_profile_enable", "cbct_profile_read", "cbct_launch_count", "cbct_device_bytes", "cbct_last_error",
 )
 
@@ -57,6 +57,8 @@ def load():
     L.cbct_bin2x2.argtypes = [vp, fp, fp, vp]
     L.cbct_energy.argtypes = [vp, fp, fp, f, f, dp, vp]
     L.cbct_fbs_reconstruct.argtypes = [vp, fp, fp, i, ip, i, f, f, f, f, fp, dp, vp]
+    L.cbct_data_gradient.argtypes = [vp, fp, fp, fp, vp]
+    L.cbct_prox_step.argtypes = [vp, fp, fp, f, f, f, f, i, fp, vp]
     L.cbct_fbs_reconstruct_until.argtypes = [vp, fp, fp, i, ip, i, f, f, f, f, f, fp, ip, vp]
     L.cbct_forward_host.argtypes = [vp, fp, fp, vp]
     L.cbct_backproject_host.argtypes = [vp, fp, fp, vp]
@@ -257,6 +259,18 @@ def fbs_reconstruct(g: Geometry, d_Y, d_f0, n_levels, n_outer, n_inner, step, mu
                                        int(n_levels), arr, int(n_inner), float(step), float(mu), float(eps),
                                        float(omega), _dev(d_f_out, g.n_vox, "d_f_out"), tr, _stream(stream)))
     return list(tr)[:total] if trace else None
+
+
+def data_gradient(g: Geometry, d_f, d_Y, d_G, stream=None):
+    """d_G = P^T (P d_f - d_Y) over this handle's angles (first half of an outer iteration)."""
+    _check(load().cbct_data_gradient(g._h, _dev(d_f, g.n_vox, "d_f"), _dev(d_Y, g.n_proj, "d_Y"), _dev(d_G, g.n_vox, "d_G"),
+                                     _stream(stream)))
+
+
+def prox_step(g: Geometry, d_f, d_G, c, beta, eps, omega, n_inner, d_f_out, stream=None):
+    """d_f_out = max(0, TVprox(d_f - c d_G)) (second half of an outer iteration)."""
+    _check(load().cbct_prox_step(g._h, _dev(d_f, g.n_vox, "d_f"), _dev(d_G, g.n_vox, "d_G"), float(c), float(beta), float(eps),
+                                 float(omega), int(n_inner), _dev(d_f_out, g.n_vox, "d_f_out"), _stream(stream)))
 
 
 def fbs_reconstruct_until(g: Geometry, d_Y, d_f0, n_levels, n_outer_max, n_inner, step, mu, eps, omega, rel_tol, d_f_out,

@@ -135,6 +135,44 @@ extern "C" cbct_status cbct_energy(const cbct_geometry *gc, const float *d_f, co
     return energy_impl(mut(gc), d_f, d_Y, mu, eps, h_out3, (cudaStream_t)stream);
 }
 
+// ---- the two halves of an outer iteration, for drivers that put an exchange step between them (NEXT-4) ----
+extern "C" cbct_status cbct_data_gradient(const cbct_geometry *gc, const float *d_f, const float *d_Y, float *d_G, void *stream)
+{
+    REQUIRE(gc && d_f && d_Y && d_G, "cbct_data_gradient: NULL argument");
+    cbct_geometry *g = mut(gc);
+    cudaStream_t st = (cudaStream_t)stream;
+    CBCT_TRY(ensure(g, &g->proj_tmp, g->n_proj(), true));
+    CBCT_TRY(op_pad_copies(g, d_f, st));
+    if (g->bp_mode == CBCT_BACKPROJECTOR_EQ2) {
+        CBCT_TRY(op_forward_padded(g, g->proj_tmp, d_Y, 2, st));
+        CBCT_TRY(ensure(g, &g->vol_a, g->n_vox()));
+        CBCT_CUDA(cudaMemsetAsync(g->vol_a, 0, g->n_vox() * sizeof(float), st));
+        // 0 - (-(dV/(du dv))) B r
+        return op_backproject_eq2(g, g->proj_tmp, g->vol_a, -(float)((g->hx * g->hy * g->hz) / (g->du * g->dv)), 0, d_G, st);
+    }
+    CBCT_TRY(op_forward_padded(g, g->proj_tmp, d_Y, 1, st));
+    CBCT_TRY(op_backproject_prefix(g, g->proj_tmp, 0, nullptr, st));
+    CBCT_TRY(op_backproject_gather(g, g->proj_tmp, st));
+    return op_combine(g, nullptr, 0.f, 0, d_G, st);
+}
+
+extern "C" cbct_status cbct_prox_step(const cbct_geometry *gc, const float *d_f, const float *d_G, float c, float beta,
+                                      float eps, float omega, int n_inner, float *d_f_out, void *stream)
+{
+    REQUIRE(gc && d_f && d_G && d_f_out, "cbct_prox_step: NULL argument");
+    REQUIRE(beta >= 0.f && eps > 0.f && omega > 0.f && n_inner >= 0, "cbct_prox_step: beta < 0, eps <= 0, omega <= 0 or n_inner < 0");
+    REQUIRE(d_G != d_f_out, "cbct_prox_step: d_f_out must not alias d_G");
+    cbct_geometry *g = mut(gc);
+    cudaStream_t st = (cudaStream_t)stream;
+    CBCT_TRY(ensure(g, &g->vol_a, g->n_vox()));
+    CBCT_TRY(op_axpy_clamp(g, d_f, d_G, c, n_inner == 0, g->vol_a, st));        // gv = f - c G (clamped if no TV step follows)
+    if (n_inner == 0) {
+        CBCT_CUDA(cudaMemcpyAsync(d_f_out, g->vol_a, g->n_vox() * sizeof(float), cudaMemcpyDeviceToDevice, st));
+        return CBCT_OK;
+    }
+    return tv_inner(g, g->vol_a, g->vol_a, d_f_out, beta, eps, omega, n_inner, 1, st);
+}
+
 // One level of Algorithm A1: f (in/out, level-sized device buffer).
 // rel_tol > 0: stop after the first iteration with ||f_new - f_old||_2 <= rel_tol ||f_new||_2 (NEXT-2; sums in fp64,
 // one stream synchronise per iteration); *iters receives the number of iterations run.

@@ -1,5 +1,7 @@
 // a7: multigrid transfers of the coarse-to-fine cascade ("multi-grid method"; O6/Q11 in DESIGN.md).
 // All HBM-bound pointwise kernels.
+#include <algorithm>
+
 #include "cbct_internal.h"
 
 namespace {
@@ -113,6 +115,27 @@ cbct_status op_clamp_copy(cbct_geometry *g, const float *in, float *out, size_t 
 {
     (void)g;
     clamp_copy_kernel<<<1184, 256, 0, st>>>(in, out, n);
+    CBCT_LAUNCH_CHECK();
+    return CBCT_OK;
+}
+
+// out = f - c G, optionally clamped at 0 (the gradient step a4 on an already summed gradient volume)
+__global__ void __launch_bounds__(256) axpy_clamp_kernel(const float *__restrict__ f, const float *__restrict__ G, float c, int clamp,
+                                                         float *__restrict__ out, size_t n)
+{
+    for (size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x; o < n; o += (size_t)gridDim.x * blockDim.x) {
+        float v = fmaf(-c, __ldg(G + o), __ldg(f + o));
+        if (clamp) v = fmaxf(v, 0.f);
+        out[o] = v;
+    }
+}
+
+cbct_status op_axpy_clamp(cbct_geometry *g, const float *f, const float *G, float c, int clamp, float *out, cudaStream_t st)
+{
+    ProfileScope ps(4, st);
+    const size_t n = g->n_vox();
+    const int blocks = (int)std::min<size_t>((n + 255) / 256, 148 * 16);
+    axpy_clamp_kernel<<<blocks, 256, 0, st>>>(f, G, c, clamp, out, n);
     CBCT_LAUNCH_CHECK();
     return CBCT_OK;
 }

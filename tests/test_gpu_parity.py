@@ -388,3 +388,56 @@ def test_short_scan_subset_reconstruction_matches_oracle(cuda_lib, dev):
     ref = fbs.fbs_reconstruct(g, Y.astype(np.float64), None, 2, [8, 8], 5, step, mu, cfg.eps, 1.0)
     assert np.linalg.norm(ref) > 0 and rel(f.cpu().numpy(), ref) <= TOL_RECON
     G.close()
+
+
+# ---- NEXT-4: the two halves of an outer iteration and the angle-sharded driver on the CUDA path ---------------
+def test_sharded_halves_and_driver(cuda_lib, dev):
+    """(1) partial data gradients over two angle shards add up to the full one; (2) the driver with one rank
+    reproduces cbct_fbs_reconstruct bit for bit; (3) two shards emulated in one process (their partial gradients
+    summed where the all-reduce would be) match the oracle's reconstruction of the full scan."""
+    import torch
+    from oracle import fbs
+    from paper_1002_3675_b200.sharded import CudaOps, fbs_reconstruct_sharded, shard_angles
+    cb = cuda_lib
+    cfg = make_config("c1")
+    g = cfg.geom
+    Y = f32(cfg.projections())
+    f0 = to_dev(f32(0.5 * cfg.volume()), dev)
+    G_all = cb.Geometry.from_synth(g)
+    d_Y = to_dev(Y, dev)
+    grad = torch.empty(G_all.vol_shape, device=dev)
+    cb.data_gradient(G_all, f0, d_Y, grad)
+    ref = o.backproject(g, o.forward(g, f0.cpu().numpy().astype(np.float64)) - Y.astype(np.float64))
+    assert rel(grad.cpu().numpy(), ref) <= TOL_OP
+    shards, part = [], torch.zeros_like(grad)
+    for r in range(2):
+        idx = shard_angles(g.n_angles, r, 2)
+        Gr = cb.Geometry.from_synth(g.with_angles(g.angles[idx]))
+        Yr = to_dev(Y[idx], dev)
+        tmp = torch.empty_like(grad)
+        cb.data_gradient(Gr, f0, Yr, tmp)
+        part += tmp
+        shards.append((Gr, Yr))
+    assert rel(part.cpu().numpy(), grad.cpu().numpy().astype(np.float64)) <= 1e-6
+    # (2) one rank
+    args = (cfg.n_inner, cfg.step, cfg.mu, cfg.eps, cfg.omega)
+    f_ref = torch.empty(G_all.vol_shape, device=dev)
+    cb.fbs_reconstruct(G_all, d_Y, None, 2, [3, 2], *args, f_ref)
+    f_one = fbs_reconstruct_sharded(CudaOps(G_all, 2), d_Y, None, 2, [3, 2], *args, g.n_angles, None)
+    torch.cuda.synchronize()
+    assert torch.equal(f_one, f_ref)
+
+    # (3) two shards in one process
+    class TwoShards(CudaOps):
+        def __init__(self):
+            self.a, self.b = CudaOps(shards[0][0], 2), CudaOps(shards[1][0], 2)
+            self.cb, self.torch, self.stream, self.levels = self.a.cb, self.a.torch, None, self.a.levels
+        def bin(self, l, Ypair): return (self.a.bin(l, Ypair[0]), self.b.bin(l, Ypair[1]))
+        def data_gradient(self, l, f, Ypair): return self.a.data_gradient(l, f, Ypair[0]) + self.b.data_gradient(l, f, Ypair[1])
+
+    f_two = fbs_reconstruct_sharded(TwoShards(), (shards[0][1], shards[1][1]), None, 2, [3, 2], *args, g.n_angles, None)
+    ref2 = fbs.fbs_reconstruct(g, Y.astype(np.float64), None, 2, [3, 2], *args)
+    assert rel(f_two.cpu().numpy(), ref2) <= TOL_RECON
+    for G_, _ in shards:
+        G_.close()
+    G_all.close()
