@@ -60,6 +60,11 @@ GEOMS = {
     "odd_dims_axis_angles": lambda: Geometry(1000., 1500., np.array([0.0, np.pi / 4, np.pi / 2, 3.0, -2.2]), 33, 21, 2.0, 2.0, 31, 29, 17, 2.0, 2.0, 2.0),
     "wide_detector_misses": lambda: Geometry(1000., 1500., equispaced_angles(5) + 0.4, 70, 45, 4.0, 6.0, 24, 24, 12, 2.0, 2.0, 2.0),
     "short_arc_200deg": lambda: Geometry(1000., 1500., np.deg2rad(np.linspace(-10.0, 190.0, 9)), 48, 40, 2.0, 2.0, 36, 36, 40, 1.5, 1.5, 1.5),
+    # detector rows 100x finer than the slices: several rays of a column cross one z plane inside a slab (the gather's loop)
+    "fine_rows_multicross": lambda: Geometry(1000., 1500., np.array([0.2, 1.9, 4.0]), 20, 2400, 3.0, 0.02, 16, 16, 16, 2.0, 2.0, 2.0),
+    # 25 detector columns per voxel row (long candidate loops), and a detector so coarse that rays skip voxel rows
+    "fine_columns": lambda: Geometry(1000., 1500., np.array([0.5, 2.4]), 600, 12, 0.12, 4.0, 16, 16, 8, 2.0, 2.0, 3.0),
+    "coarse_detector": lambda: Geometry(1000., 1500., equispaced_angles(6) + 0.1, 9, 7, 9.0, 11.0, 24, 24, 16, 1.5, 1.5, 2.0),
     "single_angle": lambda: Geometry(1000., 1500., np.array([0.77]), 40, 40, 2.0, 2.0, 32, 32, 32, 1.5, 1.5, 1.5),
 }
 
