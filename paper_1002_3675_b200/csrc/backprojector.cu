@@ -182,6 +182,7 @@ cbct_status op_backproject_prefix(cbct_geometry *g, const float *d_in, int scale
 
 cbct_status op_backproject_gather(cbct_geometry *g, const float *d_scaled, cudaStream_t st)
 {
+    // z rows per thread and slabs per CTA: compile-time tuning knobs (measured best of a sweep on B200: 16 x 4)
 #ifndef CBCT_BP_KC
 #define CBCT_BP_KC 16
 #define CBCT_BP_BI 4

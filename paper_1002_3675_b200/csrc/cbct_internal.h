@@ -172,4 +172,3 @@ cbct_status op_restrict(cbct_geometry *fine, const float *f, float *c, cudaStrea
 cbct_status op_bin2x2(cbct_geometry *fine, const float *y, float *yc, cudaStream_t st);
 cbct_status op_sumsq_diff(cbct_geometry *g, const float *a, const float *b, size_t n, double *d_out, cudaStream_t st);
 cbct_status op_axpy_clamp(cbct_geometry *g, const float *f, const float *G, float c, int clamp, float *out, cudaStream_t st);
-cbct_status op_clamp_copy(cbct_geometry *g, const float *in, float *out, size_t n, cudaStream_t st);

@@ -60,18 +60,6 @@ bin2x2_kernel(const float *__restrict__ y, float *__restrict__ yc, int nu, int n
     yc[((size_t)a * cv + v) * cu + u] = 0.25f * ((r0.x + r0.y) + (r1.x + r1.y));
 }
 
-__global__ void __launch_bounds__(256) clamp_copy_kernel(const float *__restrict__ in, float *__restrict__ out, size_t n)
-{
-    for (size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x; o < n; o += (size_t)gridDim.x * blockDim.x)
-        out[o] = fmaxf(__ldg(in + o), 0.f);
-}
-}  // namespace
-
-static cbct_status need_coarse(cbct_geometry *fine, cbct_geometry **c)
-{
-    return cbct_geometry_coarsen(fine, c, nullptr);
-}
-
 cbct_status op_prolong(cbct_geometry *fine, const float *c, float *f, cudaStream_t st)
 {
     cbct_geometry *gc;
@@ -107,14 +95,6 @@ cbct_status op_bin2x2(cbct_geometry *fine, const float *y, float *yc, cudaStream
     ProfileScope ps(6, st);
     dim3 grid((gc->nu + 255) / 256, gc->nv, gc->na);
     bin2x2_kernel<<<grid, 256, 0, st>>>(y, yc, fine->nu, fine->nv, gc->nu, gc->nv);
-    CBCT_LAUNCH_CHECK();
-    return CBCT_OK;
-}
-
-cbct_status op_clamp_copy(cbct_geometry *g, const float *in, float *out, size_t n, cudaStream_t st)
-{
-    (void)g;
-    clamp_copy_kernel<<<1184, 256, 0, st>>>(in, out, n);
     CBCT_LAUNCH_CHECK();
     return CBCT_OK;
 }

@@ -196,9 +196,6 @@ cbct_status launch_rows(cbct_geometry *g, const float *u_in, const float *gv, fl
         const long cost = ((ctas + slots - 1) / slots) * (zc + 1);
         if (best < 0 || cost < best) { best = cost; zchunk = zc; }
     }
-#ifdef CBCT_TV_ZC_FORCE
-    zchunk = CBCT_TV_ZC_FORCE;
-#endif
     dim3 grid(ytiles, (g->nz + zchunk - 1) / zchunk);
     const double hx = g->hx, hy = g->hy, hz = g->hz;
     kern<<<grid, 32 * NW, smem, st>>>(u_in, gv, u_out, g->nx, g->ny, g->nz, (float)(1.0 / (hx * hx)), (float)(1.0 / (hy * hy)),
