@@ -60,6 +60,13 @@ bin2x2_kernel(const float *__restrict__ y, float *__restrict__ yc, int nu, int n
     yc[((size_t)a * cv + v) * cu + u] = 0.25f * ((r0.x + r0.y) + (r1.x + r1.y));
 }
 
+}  // namespace
+
+static cbct_status need_coarse(cbct_geometry *fine, cbct_geometry **c)
+{
+    return cbct_geometry_coarsen(fine, c, nullptr);
+}
+
 cbct_status op_prolong(cbct_geometry *fine, const float *c, float *f, cudaStream_t st)
 {
     cbct_geometry *gc;
