@@ -38,6 +38,12 @@ def load():
         return _LIB
     path = lib_path()
     if not os.path.exists(path):
+        try:                                  # a fresh checkout: compile the CUDA path in-tree (nvcc, sm_100a); still no CPU fallback
+            from . import build as _cuda_build
+            _cuda_build.build()
+        except Exception:
+            pass
+    if not os.path.exists(path):
         raise ImportError(f"{path} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
                           "(there is no CPU fallback for the CUDA path)")
     L = C.CDLL(path)
