@@ -22,8 +22,18 @@
 // The projections handed in are pre-multiplied by the slab chord length l(u,v).
 // One launch per ray class; class 0 accumulates into a [k][x][y] array, class 1 into [k][y][x],
 // so lanes (adjacent minor index) write contiguously; op_combine() adds the two.
+#include <type_traits>
+
 #include "cbct_internal.h"
 #include "ray_common.cuh"
+
+// 1/x to 1 ulp by one MUFU instruction; denormal x is flushed to zero (the result, +-inf, is saturated by the caller)
+__device__ __forceinline__ float rcp_approx(float x)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
 
 // C[a][v][u] = sum_{v' < v} y[a][v'][u] for v = 0..nv as (sum, compensation) pairs: the rounding
 // error of every addition is carried in the second float (two-sum), so C(v2) - C(v1) evaluated as
@@ -89,7 +99,6 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
     const float sdd_du = d.sdd / d.du;
     const float hz_dv = d.hz / d.dv, dv_hz = d.dv / d.hz;
     const float zk0 = (float)(k0 - d.koff) - d.zfrac;  // plane k0 in the units of z_entry(), minus zfrac
-    const size_t cplane = (size_t)(d.nv + 1) * d.nu;
 
     for (int a = 0; a < d.na; ++a) {
         if (!angle_has[a]) continue;                   // uniform
@@ -121,45 +130,54 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
 
             const float T = fmaf(ef, r.dt, r.tc), Tn = fmaf(ef + 1.f, r.dt, r.tc);   // entry / exit ray parameter
             const float cT = hz_dv / T, cTn = hz_dv / Tn;                             // d v / d z at entry / exit
-            const float2 *Cu = C + (size_t)a * cplane + u;
-            const float *rsu = rs + (size_t)a * d.nv * d.nu + u;
+            // 32-bit element offsets of (a, v = 0, u) in the prefix sums and in the projections (checked at geometry creation)
+            const int offC = a * (d.nv + 1) * d.nu + u, offR = a * d.nv * d.nu + u;
             const float Tdv = T * dv_hz, dtdv = r.dt * dv_hz;                         // T zeta(v) = Tdv (v - cv), dt zeta(v) = dtdv (v - cv)
-            float2 c1 = make_float2(0.f, 0.f);
-            float carry = 0.f;                         // moved into the row above by the rays crossing its lower plane
+            // entry and exit bounds of a plane less than one detector row apart on every plane of the chunk: at most one
+            // ray crosses a plane inside the slab, and the loop over further crossing rays is compiled out
+            const bool single = fmaxf(fabsf(zk0), fabsf(zk0 + (float)KC)) * fabsf(cT - cTn) < 0.999f;
+            auto planes = [&](auto multi_tag) {
+                constexpr bool MULTI = decltype(multi_tag)::value;
+                float2 c1 = make_float2(0.f, 0.f);
+                float carry = 0.f;                     // moved into the row above by the rays crossing its lower plane
 #pragma unroll
-            for (int q = 0; q <= KC; ++q) {
-                // first ray at or above plane k0+q at the slab's entry / exit plane
-                const float zk = zk0 + (float)q;
-                const int vT = min(max((int)ceilf(fmaf(zk, cT, cv)), 0), d.nv);
-                const int vTn = min(max((int)ceilf(fmaf(zk, cTn, cv)), 0), d.nv);
-                const float2 c2 = __ldg(Cu + (size_t)vT * d.nu);
-                // rays crossing plane k0+q inside the slab: v in [min(vT,vTn), max(vT,vTn)).  The arithmetic of the first
-                // one runs unconditionally (its y is 0 if there is none).
-                // b = lambda at which the ray meets the plane: T(lambda) zeta(v) = zk with T(lambda) = T + lambda dt and
-                // zeta(v) = (v - cv) dv / hz, i.e. b = (zk - T zeta(v)) / (dt zeta(v)), the projector's b with its numerator
-                // taken by one FMA (a ray in the central plane, v = cv, crosses nothing; saturation turns its 0/0 into 0).
-                const int dlt = vTn - vT, vs = min(vT, vTn);
-                const float vf = (float)vs - cv;
-                const float bq = __saturatef(__fdividef(fmaf(-Tdv, vf, zk), vf * dtdv));
-                // rising iff dt zeta(v) > 0: move the sign bit of dt zeta(v) onto y
-                float yq = 0.f;
-                if (dlt != 0) yq = __ldg(rsu + (size_t)vs * d.nu);
-                yq = __int_as_float(__float_as_int(yq) ^ (__float_as_int(vf * dtdv) & 0x80000000));
-                float up = fmaxf(0.f, l1 - fmaxf(l0, bq)) * yq;       // moved up across the plane (negative: moved down)
-                if (abs(dlt) > 1) {                    // several rays cross this plane inside the slab (fine detector rows)
-                    for (int v = vs + 1; v < vs + abs(dlt); ++v) {
-                        const float b2 = __saturatef(__fdividef(fmaf(-Tdv, (float)v - cv, zk), ((float)v - cv) * dtdv));
-                        const float y2 = __ldg(rsu + (size_t)v * d.nu);
-                        up = fmaf(fmaxf(0.f, l1 - fmaxf(l0, b2)), __int_as_float(__float_as_int(y2) ^ (__float_as_int(vf * dtdv) & 0x80000000)), up);
+                for (int q = 0; q <= KC; ++q) {
+                    // first ray at or above plane k0+q at the slab's entry / exit plane
+                    const float zk = zk0 + (float)q;
+                    const int vT = min(max((int)ceilf(fmaf(zk, cT, cv)), 0), d.nv);
+                    const int vTn = min(max((int)ceilf(fmaf(zk, cTn, cv)), 0), d.nv);
+                    const float2 c2 = __ldg(C + (offC + vT * d.nu));
+                    // rays crossing plane k0+q inside the slab: v in [min(vT,vTn), max(vT,vTn)).  The arithmetic of the first
+                    // one runs unconditionally (its y is 0 if there is none).
+                    // b = lambda at which the ray meets the plane: T(lambda) zeta(v) = zk with T(lambda) = T + lambda dt and
+                    // zeta(v) = (v - cv) dv / hz, i.e. b = (zk - T zeta(v)) / (dt zeta(v)), the projector's b with its numerator
+                    // taken by one FMA (a ray in the central plane, v = cv, crosses nothing; saturation turns its 0/0 into 0).
+                    const int dlt = vTn - vT, vs = min(vT, vTn);
+                    const float vf = (float)vs - cv;
+                    const float bq = __saturatef(fmaf(-Tdv, vf, zk) * rcp_approx(vf * dtdv));
+                    // rising iff dt zeta(v) > 0: move the sign bit of dt zeta(v) onto y
+                    float yq = 0.f;
+                    if (dlt != 0) yq = __ldg(rs + (offR + vs * d.nu));
+                    yq = __int_as_float(__float_as_int(yq) ^ (__float_as_int(vf * dtdv) & 0x80000000));
+                    float up = fmaxf(0.f, l1 - fmaxf(l0, bq)) * yq;   // moved up across the plane (negative: moved down)
+                    if constexpr (MULTI) {
+                        for (int v = vs + 1; v < vs + abs(dlt); ++v) {   // further rays crossing this plane (fine detector rows)
+                            const float vf2 = (float)v - cv;
+                            const float b2 = __saturatef(fmaf(-Tdv, vf2, zk) * rcp_approx(vf2 * dtdv));
+                            const float y2 = __ldg(rs + (offR + v * d.nu));
+                            up = fmaf(fmaxf(0.f, l1 - fmaxf(l0, b2)), __int_as_float(__float_as_int(y2) ^ (__float_as_int(vf * dtdv) & 0x80000000)), up);
+                        }
                     }
+                    if (q > 0) {
+                        const float ysum = (c2.x - c1.x) + (c2.y - c1.y);
+                        acc[q > 0 ? q - 1 : 0] += fmaf(w, ysum, carry - up);
+                    }
+                    c1 = c2;
+                    carry = up;
                 }
-                if (q > 0) {
-                    const float ysum = (c2.x - c1.x) + (c2.y - c1.y);
-                    acc[q > 0 ? q - 1 : 0] += fmaf(w, ysum, carry - up);
-                }
-                c1 = c2;
-                carry = up;
-            }
+            };
+            if (single) planes(std::false_type{});
+            else planes(std::true_type{});
         }
     }
     if (!valid) return;

@@ -216,6 +216,10 @@ static cbct_status create_impl(double sad, double sdd, const double *angles, int
         cbct_set_error("cbct_geometry_create: a dimension exceeds 16384");
         return CBCT_ERR_SHAPE;
     }
+    if ((long long)na * (nv + 1) * nu >= (1LL << 31)) {
+        cbct_set_error("cbct_geometry_create: n_angles * (nv + 1) * nu must stay below 2^31 (32-bit offsets in the gather)");
+        return CBCT_ERR_SHAPE;
+    }
     const double rad = 0.5 * std::hypot(nx * hx, ny * hy);
     if (!(rad < sad) || !(rad < sdd - sad)) {
         cbct_set_error("cbct_geometry_create: the volume's circumscribed cylinder (r=%.1f mm) is not strictly "
