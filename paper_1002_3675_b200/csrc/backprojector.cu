@@ -136,16 +136,22 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
             // entry and exit bounds of a plane less than one detector row apart on every plane of the chunk: at most one
             // ray crosses a plane inside the slab, and the loop over further crossing rays is compiled out
             const bool single = fmaxf(fabsf(zk0), fabsf(zk0 + (float)KC)) * fabsf(cT - cTn) < 0.999f;
-            auto planes = [&](auto multi_tag) {
-                constexpr bool MULTI = decltype(multi_tag)::value;
+            // all run bounds of the chunk fall on the detector: no clamping needed
+            const bool inside = fminf(fminf(fmaf(zk0, cT, cv), fmaf(zk0, cTn, cv)), fminf(fmaf(zk0 + (float)KC, cT, cv), fmaf(zk0 + (float)KC, cTn, cv))) >= 0.f &&
+                                fmaxf(fmaxf(fmaf(zk0, cT, cv), fmaf(zk0, cTn, cv)), fmaxf(fmaf(zk0 + (float)KC, cT, cv), fmaf(zk0 + (float)KC, cTn, cv))) <= (float)(d.nv - 1);
+            auto planes = [&](auto multi_tag, auto clamp_tag) {
+                constexpr bool MULTI = decltype(multi_tag)::value, CLAMP = decltype(clamp_tag)::value;
                 float2 c1 = make_float2(0.f, 0.f);
                 float carry = 0.f;                     // moved into the row above by the rays crossing its lower plane
 #pragma unroll
                 for (int q = 0; q <= KC; ++q) {
                     // first ray at or above plane k0+q at the slab's entry / exit plane
                     const float zk = zk0 + (float)q;
-                    const int vT = min(max((int)ceilf(fmaf(zk, cT, cv)), 0), d.nv);
-                    const int vTn = min(max((int)ceilf(fmaf(zk, cTn, cv)), 0), d.nv);
+                    int vT = (int)ceilf(fmaf(zk, cT, cv)), vTn = (int)ceilf(fmaf(zk, cTn, cv));
+                    if constexpr (CLAMP) {
+                        vT = min(max(vT, 0), d.nv);
+                        vTn = min(max(vTn, 0), d.nv);
+                    }
                     const float2 c2 = __ldg(C + (offC + vT * d.nu));
                     // rays crossing plane k0+q inside the slab: v in [min(vT,vTn), max(vT,vTn)).  The arithmetic of the first
                     // one runs unconditionally (its y is 0 if there is none).
@@ -176,8 +182,9 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
                     carry = up;
                 }
             };
-            if (single) planes(std::false_type{});
-            else planes(std::true_type{});
+            if (single && inside) planes(std::false_type{}, std::false_type{});
+            else if (single) planes(std::false_type{}, std::true_type{});
+            else planes(std::true_type{}, std::true_type{});
         }
     }
     if (!valid) return;
