@@ -139,6 +139,7 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
             // all run bounds of the chunk fall on the detector: no clamping needed
             const bool inside = fminf(fminf(fmaf(zk0, cT, cv), fmaf(zk0, cTn, cv)), fminf(fmaf(zk0 + (float)KC, cT, cv), fmaf(zk0 + (float)KC, cTn, cv))) >= 0.f &&
                                 fmaxf(fmaxf(fmaf(zk0, cT, cv), fmaf(zk0, cTn, cv)), fmaxf(fmaf(zk0 + (float)KC, cT, cv), fmaf(zk0 + (float)KC, cTn, cv))) <= (float)(d.nv - 1);
+            const float xT0 = fmaf(zk0, cT, cv), xTn0 = fmaf(zk0, cTn, cv);          // bounds of plane k0; plane k0+q: + q cT (q a literal)
             auto planes = [&](auto multi_tag, auto clamp_tag) {
                 constexpr bool MULTI = decltype(multi_tag)::value, CLAMP = decltype(clamp_tag)::value;
                 float2 c1 = make_float2(0.f, 0.f);
@@ -147,7 +148,7 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
                 for (int q = 0; q <= KC; ++q) {
                     // first ray at or above plane k0+q at the slab's entry / exit plane
                     const float zk = zk0 + (float)q;
-                    int vT = (int)ceilf(fmaf(zk, cT, cv)), vTn = (int)ceilf(fmaf(zk, cTn, cv));
+                    int vT = (int)ceilf(fmaf((float)q, cT, xT0)), vTn = (int)ceilf(fmaf((float)q, cTn, xTn0));
                     if constexpr (CLAMP) {
                         vT = min(max(vT, 0), d.nv);
                         vTn = min(max(vTn, 0), d.nv);
