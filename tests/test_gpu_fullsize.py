@@ -116,3 +116,21 @@ def test_c5_stress_subsets(cuda_lib):
     ref = o.tv_prox(g, gv.astype(np.float64), gv.astype(np.float64), cfg.beta, cfg.eps, 1.0, 2)
     assert rel(u.cpu().numpy(), ref) <= 1e-5
     G.close()
+
+
+def test_c3_eq2_backprojector_full_size(cuda_lib):
+    """NEXT-1 at the full c3 size (512x512x64, 40 views of 512x384): the paper's eq. 2 backprojection of P(phantom)
+    against the oracle, every voxel."""
+    import torch
+    cb = cuda_lib
+    dev = torch.device("cuda:0")
+    cfg = make_config("c3")
+    g = cfg.geom
+    G = cb.Geometry.from_synth(g)
+    d_q = torch.empty(g.proj_shape, device=dev)
+    cb.forward(G, torch.from_numpy(f32(cfg.volume())).to(dev), d_q)
+    d_b = torch.empty(g.vol_shape, device=dev)
+    cb.backproject_eq2(G, d_q, d_b)
+    ref = o.backproject_eq2(g, d_q.cpu().numpy().astype(np.float64))
+    assert rel(d_b.cpu().numpy(), ref) <= 1e-5
+    G.close()
