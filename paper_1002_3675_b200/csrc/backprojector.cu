@@ -109,7 +109,7 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
             const float x = (m & 1) ? x1 : x0, y = (m & 2) ? y1 : y0;
             const float num = fmaf(-x, cs.y, y * cs.x);
             const float den = d.sad - fmaf(x, cs.x, y * cs.y);
-            const float uu = fmaf(sdd_du, __fdividef(num, den), cu);
+            const float uu = fmaf(sdd_du, num * rcp_approx(den), cu);      // den = depth of the corner > 0
             umin = fminf(umin, uu);
             umax = fmaxf(umax, uu);
         }
