@@ -443,6 +443,13 @@ def test_sharded_halves_and_driver(cuda_lib, dev):
     f_two = fbs_reconstruct_sharded(TwoShards(), (shards[0][1], shards[1][1]), None, 2, [3, 2], *args, g.n_angles, None)
     ref2 = fbs.fbs_reconstruct(g, Y.astype(np.float64), None, 2, [3, 2], *args)
     assert rel(f_two.cpu().numpy(), ref2) <= TOL_RECON
+    # argument errors of the new entry points
+    with pytest.raises(cb.CbctError) as ei:
+        cb.prox_step(G_all, f0, grad, 1e-3, 10.0, 1e-4, 1.0, 2, grad)              # output aliases the gradient
+    assert ei.value.status == 1
+    with pytest.raises(cb.CbctError) as ei:
+        cb.fbs_reconstruct_until(G_all, d_Y, None, 1, [2], *args, -1.0, f_ref)    # negative tolerance
+    assert ei.value.status == 1
     for G_, _ in shards:
         G_.close()
     G_all.close()
