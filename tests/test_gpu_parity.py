@@ -65,6 +65,9 @@ GEOMS = {
     # 25 detector columns per voxel row (long candidate loops), and a detector so coarse that rays skip voxel rows
     "fine_columns": lambda: Geometry(1000., 1500., np.array([0.5, 2.4]), 600, 12, 0.12, 4.0, 16, 16, 8, 2.0, 2.0, 3.0),
     "coarse_detector": lambda: Geometry(1000., 1500., equispaced_angles(6) + 0.1, 9, 7, 9.0, 11.0, 24, 24, 16, 1.5, 1.5, 2.0),
+    # degenerate sizes: a single slice, a single detector row, one voxel column
+    "one_slice_one_row": lambda: Geometry(1000., 1500., np.array([0.3, 2.0]), 24, 1, 2.0, 2.0, 12, 10, 1, 2.0, 2.0, 2.0),
+    "one_column": lambda: Geometry(1000., 1500., np.array([0.0, 1.0, 2.5]), 6, 30, 1.0, 1.0, 1, 1, 24, 2.0, 2.0, 1.0),
     "single_angle": lambda: Geometry(1000., 1500., np.array([0.77]), 40, 40, 2.0, 2.0, 32, 32, 32, 1.5, 1.5, 1.5),
 }
 
