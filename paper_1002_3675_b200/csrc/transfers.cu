@@ -18,18 +18,24 @@ __global__ void __launch_bounds__(256)
 prolong_kernel(const float *__restrict__ c, float *__restrict__ f, int nx, int ny, int nz,
                int cx, int cy, int cz, int ax, int ay, int az)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int j = blockIdx.y, k = blockIdx.z;
-    if (i >= nx) return;
-    int i0, i1, j0, j1, k0, k1;
-    float wi, wj, wk;
-    lin_pair(i, cx, ax, i0, i1, wi);
-    lin_pair(j, cy, ay, j0, j1, wj);
-    lin_pair(k, cz, az, k0, k1, wk);
-    auto at = [&](int kk, int jj, int ii) { return __ldg(c + ((size_t)kk * cy + jj) * cx + ii); };
-    auto lx = [&](int kk, int jj) { return fmaf(wi, at(kk, jj, i1), (1.f - wi) * at(kk, jj, i0)); };
-    auto ly = [&](int kk) { return fmaf(wj, lx(kk, j1), (1.f - wj) * lx(kk, j0)); };
-    f[((size_t)k * ny + j) * nx + i] = fmaf(wk, ly(k1), (1.f - wk) * ly(k0));
+    // a CTA takes whole (j,k) rows, a few per block, grid-strided: 4 KB of output per row instead of one tiny CTA per row
+    const int rows = ny * nz;
+    for (int row = blockIdx.x * blockDim.y + threadIdx.y; row < rows; row += gridDim.x * blockDim.y) {
+        const int j = row % ny, k = row / ny;
+        int j0, j1, k0, k1;
+        float wj, wk;
+        lin_pair(j, cy, ay, j0, j1, wj);
+        lin_pair(k, cz, az, k0, k1, wk);
+        for (int i = threadIdx.x; i < nx; i += blockDim.x) {
+            int i0, i1;
+            float wi;
+            lin_pair(i, cx, ax, i0, i1, wi);
+            auto at = [&](int kk, int jj, int ii) { return __ldg(c + ((size_t)kk * cy + jj) * cx + ii); };
+            auto lx = [&](int kk, int jj) { return fmaf(wi, at(kk, jj, i1), (1.f - wi) * at(kk, jj, i0)); };
+            auto ly = [&](int kk) { return fmaf(wj, lx(kk, j1), (1.f - wj) * lx(kk, j0)); };
+            f[((size_t)k * ny + j) * nx + i] = fmaf(wk, ly(k1), (1.f - wk) * ly(k0));
+        }
+    }
 }
 
 __global__ void __launch_bounds__(256)
@@ -73,8 +79,8 @@ cbct_status op_prolong(cbct_geometry *fine, const float *c, float *f, cudaStream
     CBCT_TRY(need_coarse(fine, &gc));
     const int *fl = fine->coarsen_flags;
     ProfileScope ps(6, st);
-    dim3 grid((fine->nx + 255) / 256, fine->ny, fine->nz);
-    prolong_kernel<<<grid, 256, 0, st>>>(c, f, fine->nx, fine->ny, fine->nz, gc->nx, gc->ny, gc->nz, fl[0], fl[1], fl[2]);
+    const int rows = fine->ny * fine->nz;
+    prolong_kernel<<<std::min((rows + 3) / 4, 148 * 16), dim3(64, 4), 0, st>>>(c, f, fine->nx, fine->ny, fine->nz, gc->nx, gc->ny, gc->nz, fl[0], fl[1], fl[2]);
     CBCT_LAUNCH_CHECK();
     return CBCT_OK;
 }
