@@ -54,7 +54,8 @@ typedef enum {
  * Builds the per-(angle,u) ray tables (fp64 on the host, stored fp32 on the device).
  * Errors: INVALID_ARG for NULL / non-positive values or sad >= sdd; SHAPE if the volume's
  * circumscribed cylinder is not strictly between source and detector, if a dimension exceeds
- * 16384, or if some ray climbs more than 0.999 voxels in z per voxel of its major (x or y) axis
+ * 16384, if a padded volume copy ((nz+4) * nx * (ny+8) elements, or with x and y swapped) or
+ * n_angles * (nv+1) * nu reaches 2^31 elements (32-bit offsets in the kernels), or if some ray climbs more than 0.999 voxels in z per voxel of its major (x or y) axis
  * (the slab march assumes at most one z-plane crossing per slab; true for every cone-beam CT
  * geometry with hz not much smaller than hx, hy).  No device memory is touched if this fails.
  */
