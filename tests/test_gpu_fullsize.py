@@ -134,3 +134,21 @@ def test_c3_eq2_backprojector_full_size(cuda_lib):
     ref = o.backproject_eq2(g, d_q.cpu().numpy().astype(np.float64))
     assert rel(d_b.cpu().numpy(), ref) <= 1e-5
     G.close()
+
+
+def test_c5_coarsest_level_two_outer_iterations(cuda_lib):
+    """c5's loop: the full-size oracle is infeasible, so the first 2 outer iterations at the size
+    of its coarsest level (128^3 voxels of 2 mm, 360 views of 256x192, the same scene) against the oracle."""
+    import torch
+    cb = cuda_lib
+    dev = torch.device("cuda:0")
+    cfg = make_config("c5", shrink=4)
+    g = cfg.geom
+    assert (g.nx, g.ny, g.nz, g.n_angles, g.nu, g.nv) == (128, 128, 128, 360, 256, 192)
+    G = cb.Geometry.from_synth(g)
+    Y = f32(cfg.projections())
+    f = torch.empty(g.vol_shape, device=dev)
+    cb.fbs_reconstruct(G, torch.from_numpy(Y).to(dev), None, 1, [2], cfg.n_inner, cfg.step, cfg.mu, cfg.eps, cfg.omega, f)
+    ref = o.fbs_reconstruct(g, Y.astype(np.float64), None, 1, [2], cfg.n_inner, cfg.step, cfg.mu, cfg.eps, cfg.omega)
+    assert np.linalg.norm(ref) > 0 and rel(f.cpu().numpy(), ref) <= 1e-4
+    G.close()
