@@ -129,7 +129,7 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
             if (!(w > 0.f)) continue;
 
             const float T = fmaf(ef, r.dt, r.tc), Tn = fmaf(ef + 1.f, r.dt, r.tc);   // entry / exit ray parameter
-            const float cT = hz_dv / T, cTn = hz_dv / Tn;                             // d v / d z at entry / exit
+            const float cT = hz_dv * rcp_approx(T), cTn = hz_dv * rcp_approx(Tn);     // d v / d z at entry / exit (T > 0)
             // 32-bit element offsets of (a, v = 0, u) in the prefix sums and in the projections (checked at geometry creation)
             const int offC = a * (d.nv + 1) * d.nu + u, offR = a * d.nv * d.nu + u;
             const float Tdv = T * dv_hz, dtdv = r.dt * dv_hz;                         // T zeta(v) = Tdv (v - cv), dt zeta(v) = dtdv (v - cv)
