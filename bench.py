@@ -157,8 +157,7 @@ def run_gpu(args):
 
     cfg = make_config("c2")
     g = cfg.geom
-    # replicas: every rank reconstructs its own independent scan (different noise-free data set per rank
-    # would be identical here, so ranks differ only by the start volume seed); no data-path collective
+    # replicas only: every rank runs its own copy of the same seeded scan; no data-path collective
     Y = np.ascontiguousarray(cfg.projections(), dtype=np.float32)
     G = cb.Geometry.from_synth(g)
     n_outer = [1] * LEVELS
