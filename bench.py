@@ -35,6 +35,8 @@ METRIC = "projector+backprojector GUPS (voxel-projection updates/s of P and P^T 
 UNIT = "GUPS"
 N_INNER = 10
 LEVELS = 2
+TRAFFIC_COVERS = ("dram__bytes_read.sum + dram__bytes_write.sum of ONE fine-level launch of the dominant kernel "
+                  "(profiles/traffic.csv, from the committed ncu --set full capture)")
 LANE_OPS_PER_CHORD = 16          # issue-bound model of the exact-chord march/gather
 NNZ = {"c2": 2.45e9, "c3": 3.85e9}   # chords per application of P; refined by frozen_params.json
 
@@ -256,12 +258,14 @@ def run_gpu(args):
         pass
     if dom == "tv_sweep":
         roof = {"kernel": "tv_sweep_kernel", "bound": "hbm", "achieved": tv_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s",
-                "frac": tv_gbs / pk["hbm_gbs"], "traffic": traffic, "peak_source": pk["which"]}
+                "frac": tv_gbs / pk["hbm_gbs"], "traffic": traffic, "traffic_covers": TRAFFIC_COVERS,
+                "peak_source": "MEASURED_PEAKS.json copy bandwidth" if pk["which"] == "measured" else "fallback (B200_PROFILING.md)"}
     else:
         peak = sm_count * 128 * pk["sm_max_mhz"] * 1e6 / 1e12            # T lane-op/s (fp32 issue: SMs x 128 lanes x clock)
         ach = LANE_OPS_PER_CHORD * nnz_step / (per_step_ms(dom) / 1e3) / 1e12
         roof = {"kernel": dom + "_kernel", "bound": "alu", "achieved": ach, "peak": peak, "unit": "Tlane-op/s",
-                "frac": ach / peak, "traffic": traffic, "peak_source": pk["which"],
+                "frac": ach / peak, "traffic": traffic, "traffic_covers": TRAFFIC_COVERS,
+                "peak_source": f"nominal lanes ({sm_count} SMs x 128 fp32 lanes) x max SM clock ({pk['sm_max_mhz']:.0f} MHz, {pk['which']})",
                 "model": f"{LANE_OPS_PER_CHORD} fp32 lane-ops per chord x {nnz_step:.3e} chords per step (SURVEY.md 8(d))",
                 "chords_per_s": nnz_step / (per_step_ms(dom) / 1e3)}
 
@@ -438,6 +442,21 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def launch_ranks(n: int) -> int:
+    """`bench.py --gpus N` started by hand (no RANK in the environment): re-run this command as N ranks, one per GPU, under
+    torch.distributed.run on this node (rendezvous on 127.0.0.1, a free port), exactly as the driver launches it."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")                       # the communicator log shows the ranks (and NVLS, if used)
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd, env=env)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -449,8 +468,16 @@ def main():
     ap.add_argument("--cpu-angles", type=int, default=8)
     ap.add_argument("--shard-angles", action="store_true",
                     help="NEXT-4: shard the views of ONE reconstruction over the ranks (strong scaling) instead of replicas")
+    ap.add_argument("--rank-probe", action="store_true",
+                    help="every rank prints its RANK/LOCAL_RANK/WORLD_SIZE and exits (checks the launcher without a GPU)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
+    if args.gpus > 1 and "RANK" not in os.environ and args.impl == "cuda":
+        raise SystemExit(launch_ranks(args.gpus))              # one process per GPU; rank 0 prints the JSON line
+    if args.rank_probe:
+        print(json.dumps({k: os.environ.get(k) for k in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+                         | {"mode": "shard-angles" if args.shard_angles else "replicas"}), flush=True)
+        return
     if args.impl == "reference":
         run_reference(args)
     elif args.shard_angles:

@@ -49,12 +49,17 @@ class Config:
         return ph.line_integrals(self.ells, self.geom, angle_indices)
 
     def projections(self, angle_indices=None) -> np.ndarray:
-        """The observed data Y: analytic line integrals, Poisson/log noise if I0 is set."""
+        """The observed data Y: analytic line integrals, Poisson/log noise if I0 is set.  Every view draws its
+        noise from its own stream seeded by (config seed, view index), so a subset of the views (an angle shard of
+        a multi-GPU run, a sampled sub-problem) is exactly that part of the one full noisy scan."""
         p = self.clean_projections(angle_indices)
         if self.I0 is None:
             return p
-        rng = np.random.default_rng(self.seed + 7919)
-        return ph.poisson_log(p, self.I0, rng)
+        idx = range(self.geom.n_angles) if angle_indices is None else list(angle_indices)
+        out = np.empty_like(p)
+        for n, ia in enumerate(idx):
+            out[n] = ph.poisson_log(p[n], self.I0, np.random.default_rng([self.seed + 7919, int(ia)]))
+        return out
 
 
 def s_max_estimate(g: Geometry) -> float:

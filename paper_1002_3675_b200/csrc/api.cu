@@ -30,7 +30,7 @@ extern "C" cbct_status cbct_backproject(const cbct_geometry *gc, const float *d_
     REQUIRE(gc && d_proj && d_vol, "cbct_backproject: NULL argument");
     cbct_geometry *g = mut(gc);
     cudaStream_t st = (cudaStream_t)stream;
-    CBCT_TRY(ensure(g, &g->proj_tmp, g->n_proj(), true));
+    CBCT_TRY(ensure_zeroed(g, &g->proj_tmp, g->n_proj(), st));
     CBCT_TRY(op_backproject_prefix(g, d_proj, 1, g->proj_tmp, st));       // l * y and its prefix sums along v
     CBCT_TRY(op_backproject_gather(g, g->proj_tmp, st));
     return op_combine(g, nullptr, 0.f, 0, d_vol, st);
@@ -46,7 +46,7 @@ extern "C" cbct_status cbct_set_backprojector(cbct_geometry *g, int mode)
 {
     REQUIRE(g, "cbct_set_backprojector: NULL handle");
     REQUIRE(mode == CBCT_BACKPROJECTOR_EXACT || mode == CBCT_BACKPROJECTOR_EQ2, "cbct_set_backprojector: unknown mode %d", mode);
-    g->bp_mode = mode;
+    for (cbct_geometry *q = g; q; q = q->coarse) q->bp_mode = mode;      // coarse levels created later inherit it (cbct_geometry_coarsen)
     return CBCT_OK;
 }
 
@@ -110,7 +110,7 @@ extern "C" cbct_status cbct_bin2x2(const cbct_geometry *fine, const float *y, fl
 static cbct_status energy_impl(cbct_geometry *g, const float *d_f, const float *d_Y, float mu, float eps,
                                double *out3, cudaStream_t st)
 {
-    CBCT_TRY(ensure(g, &g->proj_tmp, g->n_proj(), true));
+    CBCT_TRY(ensure_zeroed(g, &g->proj_tmp, g->n_proj(), st));
     CBCT_TRY(ensure(g, &g->red_out, (size_t)2));
     if (!g->h_red) CBCT_CUDA(cudaMallocHost((void **)&g->h_red, 2 * sizeof(double)));
     CBCT_TRY(op_pad_copies(g, d_f, st));
@@ -141,7 +141,7 @@ extern "C" cbct_status cbct_data_gradient(const cbct_geometry *gc, const float *
     REQUIRE(gc && d_f && d_Y && d_G, "cbct_data_gradient: NULL argument");
     cbct_geometry *g = mut(gc);
     cudaStream_t st = (cudaStream_t)stream;
-    CBCT_TRY(ensure(g, &g->proj_tmp, g->n_proj(), true));
+    CBCT_TRY(ensure_zeroed(g, &g->proj_tmp, g->n_proj(), st));
     CBCT_TRY(op_pad_copies(g, d_f, st));
     if (g->bp_mode == CBCT_BACKPROJECTOR_EQ2) {
         CBCT_TRY(op_forward_padded(g, g->proj_tmp, d_Y, 2, st));
@@ -185,7 +185,7 @@ static cbct_status fbs_level(cbct_geometry *g, const float *d_Y, float *f, int n
         if (!g->h_red) CBCT_CUDA(cudaMallocHost((void **)&g->h_red, 2 * sizeof(double)));
     }
     if (iters) *iters = 0;
-    CBCT_TRY(ensure(g, &g->proj_tmp, g->n_proj(), true));
+    CBCT_TRY(ensure_zeroed(g, &g->proj_tmp, g->n_proj(), st));
     CBCT_TRY(ensure(g, &g->vol_a, g->n_vox()));
     const float beta = mu / step;
     const float c = (float)(2.0 * (double)step * (double)g->n_vox() / ((double)g->na * g->nu * g->nv));
@@ -247,7 +247,6 @@ static cbct_status fbs_cascade(const cbct_geometry *gc, const float *d_Y, const 
     lev[0] = mut(gc);
     for (int l = 1; l < n_levels; ++l) {
         CBCT_TRY(cbct_geometry_coarsen(lev[l - 1], &lev[l], nullptr));
-        lev[l]->bp_mode = lev[0]->bp_mode;
     }
 
     // data per level: level 0 uses d_Y, coarser levels their own binned copy

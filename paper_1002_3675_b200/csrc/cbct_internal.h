@@ -132,12 +132,19 @@ struct ProfileScope {
 };
 
 // ---- scratch ------------------------------------------------------------------------------
-cbct_status cbct_dev_alloc(cbct_geometry *g, void **p, size_t bytes, bool zero);
+// zero = true clears the new buffer with cudaMemsetAsync on `st`, the stream of the first kernel that will use it
+cbct_status cbct_dev_alloc(cbct_geometry *g, void **p, size_t bytes, bool zero, cudaStream_t st);
 template <typename T>
-inline cbct_status ensure(cbct_geometry *g, T **p, size_t count, bool zero = false)
+inline cbct_status ensure(cbct_geometry *g, T **p, size_t count)
 {
     if (*p) return CBCT_OK;
-    return cbct_dev_alloc(g, (void **)p, count * sizeof(T), zero);
+    return cbct_dev_alloc(g, (void **)p, count * sizeof(T), false, nullptr);
+}
+template <typename T>
+inline cbct_status ensure_zeroed(cbct_geometry *g, T **p, size_t count, cudaStream_t st)
+{
+    if (*p) return CBCT_OK;
+    return cbct_dev_alloc(g, (void **)p, count * sizeof(T), true, st);
 }
 inline size_t pad_elems(const cbct_geometry *g, int c)
 {

@@ -21,7 +21,7 @@ void cbct_set_error(const char *fmt, ...)
 extern "C" const char *cbct_last_error(void) { return t_err; }
 extern "C" unsigned long long cbct_launch_count(void) { return g_cbct_launches; }
 
-cbct_status cbct_dev_alloc(cbct_geometry *g, void **p, size_t bytes, bool zero)
+cbct_status cbct_dev_alloc(cbct_geometry *g, void **p, size_t bytes, bool zero, cudaStream_t st)
 {
     cudaError_t e = cudaMalloc(p, bytes);
     if (e != cudaSuccess) {
@@ -30,7 +30,9 @@ cbct_status cbct_dev_alloc(cbct_geometry *g, void **p, size_t bytes, bool zero)
         cbct_set_error("cudaMalloc(%zu bytes) failed: %s", bytes, cudaGetErrorString(e));
         return CBCT_ERR_ALLOC;
     }
-    if (zero) CBCT_CUDA(cudaMemset(*p, 0, bytes));
+    // zero-fill ON THE CALLER'S STREAM: the first kernel that touches the buffer is launched on it right afterwards,
+    // and nothing orders the legacy default stream against a non-blocking stream (PyTorch's side streams)
+    if (zero) CBCT_CUDA(cudaMemsetAsync(*p, 0, bytes, st));
     g->bytes += bytes;
     return CBCT_OK;
 }
@@ -75,7 +77,7 @@ template <typename T>
 static cbct_status upload(cbct_geometry *g, T **dst, const std::vector<T> &src)
 {
     if (src.empty()) { *dst = nullptr; return CBCT_OK; }
-    CBCT_TRY(cbct_dev_alloc(g, (void **)dst, src.size() * sizeof(T), false));
+    CBCT_TRY(cbct_dev_alloc(g, (void **)dst, src.size() * sizeof(T), false, nullptr));
     CBCT_CUDA(cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice));
     return CBCT_OK;
 }
@@ -171,11 +173,12 @@ static cbct_status build_tables(cbct_geometry *g)
         }
         for (int c = 0; c < 2; ++c)
             for (int u0 = 0; u0 < nu; u0 += 32) {
+                // every ray is written by exactly one launch (the one of its class), whether it meets the volume or
+                // not: a tile is listed for class c as soon as it holds a ray of class c, so rays that miss still get
+                // their 0 (mode 0) or -Y (residual modes) and nothing stale survives in the output
                 bool any = false;
-                for (int u = u0; u < u0 + 32 && u < nu; ++u) {
-                    const RayXY &r = rays[(size_t)a * nu + u];
-                    if (ray_cls(r.range) == c && ray_ihi(r.range) > ray_ilo(r.range)) any = true;
-                }
+                for (int u = u0; u < u0 + 32 && u < nu; ++u)
+                    if (ray_cls(rays[(size_t)a * nu + u].range) == c) any = true;
                 if (any) tiles[c].push_back(make_int2(a, u0));
             }
     }
@@ -196,6 +199,9 @@ static cbct_status build_tables(cbct_geometry *g)
         CBCT_TRY(upload(g, &g->d_angle_has[c], g->h_angle_has[c]));
     }
     d.rays = g->d_rays; d.cs = g->d_cs; d.zeta = g->d_zeta; d.inv_zeta = g->d_inv_zeta; d.dz_mm = g->d_dz;
+    // the table uploads are cudaMemcpy's from pageable memory on the legacy default stream: wait for them here, so that the
+    // first kernel may run on any (also a non-blocking) stream
+    CBCT_CUDA(cudaStreamSynchronize(nullptr));
     return CBCT_OK;
 }
 
@@ -282,6 +288,7 @@ extern "C" cbct_status cbct_geometry_coarsen(const cbct_geometry *gc, cbct_geome
         cbct_geometry *c = nullptr;
         CBCT_TRY(create_impl(g->sad, g->sdd, g->angles.data(), g->na, nu, nv, du, dv, n[0], n[1], n[2],
                              hn[0], hn[1], hn[2], &c));
+        c->bp_mode = g->bp_mode;
         g->coarse = c;
         std::memcpy(g->coarsen_flags, fl, sizeof(fl));
     }

@@ -43,7 +43,7 @@ __global__ void __launch_bounds__(256) pad_copy_kernel(const float *__restrict__
 cbct_status op_pad_copies(cbct_geometry *g, const float *d_vol, cudaStream_t st)
 {
     for (int c = 0; c < 2; ++c)
-        if (g->n_tiles[c] > 0) CBCT_TRY(ensure(g, &g->vol_pad[c], pad_elems(g, c), true));
+        if (g->n_tiles[c] > 0) CBCT_TRY(ensure_zeroed(g, &g->vol_pad[c], pad_elems(g, c), st));
     float *px = g->n_tiles[0] > 0 ? g->vol_pad[0] : nullptr;
     float *py = g->n_tiles[1] > 0 ? g->vol_pad[1] : nullptr;
     if (!px && !py) return CBCT_OK;
@@ -183,8 +183,8 @@ cbct_status op_forward_padded(cbct_geometry *g, float *d_out, const float *d_Y, 
 #endif
     constexpr int V = CBCT_FW_V, WARPS = CBCT_FW_WARPS;
     ProfileScope ps(1, st);
-    // rays in no tile miss the volume: P f = 0 there
-    if (mode == 0) CBCT_CUDA(cudaMemsetAsync(d_out, 0, g->n_proj() * sizeof(float), st));
+    // every ray belongs to a tile of its class (geometry.cu), so every output element is written: 0 / -Y / -l Y for a
+    // ray that misses the volume
     for (int c = 0; c < 2; ++c) {
         if (g->n_tiles[c] == 0) continue;
         dim3 grid(g->n_tiles[c], (g->nv + V * WARPS - 1) / (V * WARPS)), block(32, WARPS);

@@ -19,12 +19,12 @@ def rel(a, b):
     return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
 
 
-def sampled_operator_parity(cb, cfg, n_rays=4000, n_vox=600, angle_subset=None, adjoint=True):
+def sampled_operator_parity(cb, cfg, n_rays=4000, n_vox=600, angle_subset=None, adjoint=True, vol=None):
     import torch
     dev = torch.device("cuda:0")
     g = cfg.geom if angle_subset is None else cfg.geom.with_angles(cfg.geom.angles[angle_subset])
     G = cb.Geometry.from_synth(g)
-    vol = f32(cfg.volume())
+    vol = f32(cfg.volume()) if vol is None else vol
     d_vol = torch.from_numpy(vol).to(dev)
     d_q = torch.empty(g.proj_shape, device=dev)
     cb.forward(G, d_vol, d_q)
@@ -96,20 +96,61 @@ def test_c3_one_full_size_outer_iteration(cuda_lib):
     G.close()
 
 
-def test_c5_stress_subsets(cuda_lib):
-    """c5 (512^3, 360 views of 1024x768): operator parity on a fixed 8-angle subset (row blocks of P and
-    partial sums of P^T are exact sub-problems), TV parity on the full volume."""
+@pytest.mark.parametrize("name,n_outer", [("c3", [15, 15]), ("c4", [25, 25, 25])])
+def test_full_size_cascade_many_iterations(cuda_lib, name, n_outer):
+    """The c3 / c4 cascades at their FULL sizes (512x512x64, 40 / 20 noisy views of 512x384, all multigrid levels), with
+    enough outer iterations per level to see the fp32 error accumulate (the full 100 per level run once under
+    CBCT_FULL_COUNT=1, tests/test_gpu_fullcount.py; its growth table is in DESIGN.md)."""
     import torch
     cb = cuda_lib
     dev = torch.device("cuda:0")
-    cfg = make_config("c5")
-    subset = np.arange(0, 360, 45) + 3
-    e_fwd, e_bp, e_adj = sampled_operator_parity(cb, cfg, n_rays=3000, n_vox=400, angle_subset=subset)
+    cfg = make_config(name)
+    g = cfg.geom
+    G = cb.Geometry.from_synth(g)
+    Y = f32(cfg.projections())
+    f = torch.empty(g.vol_shape, device=dev)
+    cb.fbs_reconstruct(G, torch.from_numpy(Y).to(dev), None, cfg.n_levels, n_outer, cfg.n_inner, cfg.step, cfg.mu, cfg.eps,
+                       cfg.omega, f)
+    ref = o.fbs_reconstruct(g, Y.astype(np.float64), None, cfg.n_levels, n_outer, cfg.n_inner, cfg.step, cfg.mu, cfg.eps,
+                            cfg.omega)
+    out = f.cpu().numpy()
+    assert np.linalg.norm(ref) > 0 and rel(out, ref) <= 1e-4
+    assert out.min() >= 0.0
+    G.close()
+
+
+_C5 = {}
+
+
+def c5_config():
+    if "cfg" not in _C5:
+        _C5["cfg"] = make_config("c5")
+        _C5["vol"] = f32(_C5["cfg"].volume())
+    return _C5["cfg"]
+
+
+@pytest.mark.parametrize("first", [3, 0, 17, 31])
+def test_c5_operator_subsets(cuda_lib, first):
+    """c5 (512^3, 360 views of 1024x768): operator parity on 8-angle subsets {first + 45 m} (row blocks of P and partial
+    sums of P^T are exact sub-problems).  first = 0 holds the axis-aligned views and the 45-degree views where the ray class
+    changes inside a projection."""
+    cfg = c5_config()
+    subset = np.arange(0, 360, 45) + first
+    e_fwd, e_bp, e_adj = sampled_operator_parity(cuda_lib, cfg, n_rays=3000, n_vox=400, angle_subset=subset, vol=_C5["vol"])
+    print(f"c5 subset {first}: forward {e_fwd:.2e} backproject {e_bp:.2e} adjoint {e_adj:.2e}")
     assert e_fwd <= 1e-5 and e_bp <= 1e-5 and e_adj <= 1e-5, (e_fwd, e_bp, e_adj)
+
+
+def test_c5_tv_full_volume(cuda_lib):
+    """TV parity on the full 512^3 volume."""
+    import torch
+    cb = cuda_lib
+    dev = torch.device("cuda:0")
+    cfg = c5_config()
     g = cfg.geom.with_angles(cfg.geom.angles[:1])
     G = cb.Geometry.from_synth(g)
     rng = np.random.default_rng(77)
-    gv = f32(cfg.volume() + 0.002 * rng.standard_normal(g.vol_shape, dtype=np.float32))
+    gv = f32(_C5["vol"] + 0.002 * rng.standard_normal(g.vol_shape, dtype=np.float32))
     d_g = torch.from_numpy(gv).to(dev)
     u = d_g.clone()
     cb.tv_prox(G, d_g, u, cfg.beta, cfg.eps, 1.0, 2)

@@ -69,6 +69,10 @@ GEOMS = {
     "one_slice_one_row": lambda: Geometry(1000., 1500., np.array([0.3, 2.0]), 24, 1, 2.0, 2.0, 12, 10, 1, 2.0, 2.0, 2.0),
     "one_column": lambda: Geometry(1000., 1500., np.array([0.0, 1.0, 2.5]), 6, 30, 1.0, 1.0, 1, 1, 24, 2.0, 2.0, 1.0),
     "single_angle": lambda: Geometry(1000., 1500., np.array([0.77]), 40, 40, 2.0, 2.0, 32, 32, 32, 1.5, 1.5, 1.5),
+    # odd nv with even nz: the central detector row lies exactly in the voxel plane k = nz/2 (reading Q15: it belongs to the
+    # row above); 40 detector rows per slice, so the run bounds of that plane sit in a higher binade than the row index
+    "odd_rows_even_slices": lambda: Geometry(1000., 1500., np.array([0.1, 0.9, 2.3, 4.4]), 24, 401, 2.5, 0.05, 20, 20, 16, 2.0, 2.0, 2.0),
+    "odd_rows_even_slices_coarse": lambda: Geometry(1000., 1500., equispaced_angles(5) + 0.05, 40, 33, 2.0, 2.0, 24, 24, 12, 2.0, 2.0, 2.0),
 }
 
 
@@ -127,7 +131,12 @@ def test_backproject_of_unit_projections_matches_brute_force_clip(cuda_lib, dev)
     G.close()
 
 
-@pytest.mark.parametrize("shape,h", [((64, 48, 40), (0.5, 0.5, 2.5)), ((33, 21, 10), (1.0, 2.0, 0.7)), ((8, 8, 8), (1.0, 1.0, 1.0))])
+@pytest.mark.parametrize("shape,h", [((64, 48, 40), (0.5, 0.5, 2.5)), ((33, 21, 10), (1.0, 2.0, 0.7)), ((8, 8, 8), (1.0, 1.0, 1.0)),
+                                     # every instantiation of the row kernel: scalar rows (nx % 4 != 0) of 4, 8 and 16 voxels
+                                     # per lane, vector rows of 4, 8, 16; and the tile kernel for nx > 512 (ragged and full tiles)
+                                     ((102, 9, 7), (1.0, 1.0, 2.0)), ((130, 7, 6), (0.5, 0.5, 2.5)), ((258, 6, 5), (1.0, 1.0, 1.0)),
+                                     ((100, 13, 9), (1.0, 1.0, 1.0)), ((200, 11, 5), (1.0, 1.0, 1.0)), ((512, 12, 6), (0.5, 0.5, 2.5)),
+                                     ((516, 10, 9), (1.0, 1.0, 1.0)), ((1024, 9, 10), (0.5, 0.5, 0.5))])
 def test_tv_prox(cuda_lib, dev, shape, h):
     import torch
     cb = cuda_lib
@@ -396,6 +405,81 @@ def test_short_scan_subset_reconstruction_matches_oracle(cuda_lib, dev):
     ref = fbs.fbs_reconstruct(g, Y.astype(np.float64), None, 2, [8, 8], 5, step, mu, cfg.eps, 1.0)
     assert np.linalg.norm(ref) > 0 and rel(f.cpu().numpy(), ref) <= TOL_RECON
     G.close()
+
+
+def test_eq2_loop_writes_the_residual_of_rays_that_miss(cuda_lib, dev):
+    """Step 1 with eq. 2 on a detector much wider than the volume's shadow, with data that is NOT zero outside
+    the shadow: the residual of a ray that misses the volume is -Y, and eq. 2's bilinear fetch reads such pixels for voxels at
+    the lateral edge.  The handle first runs a backprojection, so its residual scratch holds other values beforehand."""
+    import torch
+    from oracle import fbs
+    from cbct_synth.configs import s_max_estimate
+    cb = cuda_lib
+    cases = {"wide_detector_misses": (GEOMS["wide_detector_misses"](), 1, [4]),
+             "wide_even_2_levels": (Geometry(1000., 1500., equispaced_angles(5) + 0.4, 72, 44, 4.0, 6.0, 24, 24, 12, 2.0, 2.0, 2.0), 2, [2, 3]),
+             "coarse_detector": (GEOMS["coarse_detector"](), 1, [4])}
+    for name, (g, nl, n_outer) in cases.items():
+        G = cb.Geometry.from_synth(g)
+        rng = np.random.default_rng(31)
+        vol = f32(smooth_phantom(g, 3))
+        Y = f32(o.forward(g, vol.astype(np.float64)) + 0.3 + 0.1 * rng.random(g.proj_shape))
+        step = 0.5 * s_max_estimate(g)
+        eps = 1e-3
+        mu = step * 4.0 * (1 / g.hx ** 2 + 1 / g.hy ** 2 + 1 / g.hz ** 2) / eps
+        junk = torch.empty(G.vol_shape, device=dev)
+        cb.backproject(G, to_dev(7.0 + rng.random(g.proj_shape), dev), junk)         # leaves l*y in the scratch projections
+        for mode, bp in ((cb.BACKPROJECTOR_EQ2, "eq2"), (cb.BACKPROJECTOR_EXACT, "exact")):
+            cb.set_backprojector(G, mode)
+            f = torch.empty(G.vol_shape, device=dev)
+            cb.fbs_reconstruct(G, to_dev(Y, dev), to_dev(vol, dev), nl, n_outer, 3, step, mu, eps, 1.0, f)
+            ref = fbs.fbs_reconstruct(g, Y.astype(np.float64), vol.astype(np.float64), nl, n_outer, 3, step, mu, eps, 1.0, backprojector=bp)
+            assert np.linalg.norm(ref) > 0 and rel(f.cpu().numpy(), ref) <= TOL_RECON, (name, bp)
+            # the data gradient alone (no prox in between): every residual pixel counts
+            Gd = torch.empty(G.vol_shape, device=dev)
+            cb.data_gradient(G, to_dev(vol, dev), to_dev(Y, dev), Gd)
+            r = o.forward(g, vol.astype(np.float64)) - Y.astype(np.float64)
+            gref = o.backproject(g, r) if bp == "exact" else (g.hx * g.hy * g.hz / (g.du * g.dv)) * o.backproject_eq2(g, r)
+            assert rel(Gd.cpu().numpy(), gref) <= TOL_OP, (name, bp)
+        G.close()
+
+
+def test_first_call_on_a_side_stream(cuda_lib, dev):
+    """The handle allocates and zero-fills its scratch (padded volume copies, scratch projections) on first use: that must be
+    ordered on the CALLER'S stream.  Every first call here runs on a fresh non-blocking torch stream while the legacy default
+    stream is kept busy."""
+    import torch
+    cb = cuda_lib
+    cfg = make_config("c2", shrink=2)
+    g = cfg.geom
+    vol = f32(cfg.volume())
+    q_ref = o.forward(g, vol.astype(np.float64))
+    busy = torch.empty(64 << 20, device=dev)
+    for first in ("forward", "fbs", "backproject"):
+        G = cb.Geometry.from_synth(g)
+        st = torch.cuda.Stream(device=dev)
+        d_vol = to_dev(vol, dev)
+        q = torch.empty(G.proj_shape, device=dev)
+        b = torch.empty(G.vol_shape, device=dev)
+        torch.cuda.synchronize()
+        for _ in range(4):
+            busy.add_(1.0)                                   # work on the default stream around the first call
+        with torch.cuda.stream(st):
+            if first == "forward":
+                cb.forward(G, d_vol, q, stream=st)
+                st.synchronize()
+                assert rel(q.cpu().numpy(), q_ref) <= TOL_OP
+            elif first == "backproject":
+                cb.backproject(G, to_dev(q_ref, dev), b, stream=st)
+                st.synchronize()
+                assert rel(b.cpu().numpy(), o.backproject(g, f32(q_ref).astype(np.float64))) <= TOL_OP
+            else:
+                Y = f32(cfg.projections())
+                cb.fbs_reconstruct(G, to_dev(Y, dev), None, 2, [1, 1], 4, cfg.step, cfg.mu, cfg.eps, 1.0, b, stream=st)
+                st.synchronize()
+                ref = o.fbs_reconstruct(g, Y.astype(np.float64), None, 2, [1, 1], 4, cfg.step, cfg.mu, cfg.eps, 1.0)
+                assert rel(b.cpu().numpy(), ref) <= TOL_RECON
+        torch.cuda.synchronize()
+        G.close()
 
 
 # ---- NEXT-4: the two halves of an outer iteration and the angle-sharded driver on the CUDA path ---------------

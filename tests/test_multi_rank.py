@@ -117,3 +117,24 @@ def test_angle_sharded_driver_equals_the_single_rank_reconstruction():
     # the partition covers every angle exactly once
     idx = np.sort(np.concatenate([shard_angles(17, r, 3) for r in range(3)]))
     assert np.array_equal(idx, np.arange(17))
+
+
+def test_bench_gpus_n_starts_n_ranks_by_itself():
+    """`python bench.py --gpus 2` with no RANK in the environment re-runs itself as 2 ranks under torch.distributed.run
+    (replicas and --shard-angles alike); --rank-probe makes every rank print its environment instead of touching a GPU."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    for extra, mode in (([], "replicas"), (["--shard-angles"], "shard-angles")):
+        r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--rank-probe"] + extra,
+                           capture_output=True, text=True, env=env, timeout=300)
+        assert r.returncode == 0, r.stderr[-2000:]
+        rows = [json.loads(l) for l in r.stdout.splitlines() if l.startswith("{")]
+        assert sorted(x["RANK"] for x in rows) == ["0", "1"]
+        assert sorted(x["LOCAL_RANK"] for x in rows) == ["0", "1"]
+        assert all(x["WORLD_SIZE"] == "2" and x["MASTER_ADDR"] == "127.0.0.1" and x["mode"] == mode for x in rows)
+    # under a launcher (RANK set) the command does not spawn again
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--rank-probe"], capture_output=True,
+                       text=True, env=dict(env, RANK="1", LOCAL_RANK="1", WORLD_SIZE="2"), timeout=120)
+    rows = [json.loads(l) for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(rows) == 1 and rows[0]["RANK"] == "1"
