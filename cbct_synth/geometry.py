@@ -5,7 +5,9 @@ Lengths are mm.  Rotation axis is z.  For projection angle theta:
   source          S = (SAD cos t, SAD sin t, 0)
   detector centre C = -(SDD - SAD) (cos t, sin t, 0)
   detector axes   u^ = (-sin t, cos t, 0),  v^ = (0, 0, 1)
-  pixel (iu, iv) centre  D = C + (iu-(nu-1)/2) du u^ + (iv-(nv-1)/2) dv v^
+  pixel (iu, iv) centre  D = C + ((iu-(nu-1)/2) du + off_u) u^ + ((iv-(nv-1)/2) dv + off_v) v^
+  (off_u, off_v: in-plane shift of the detector panel in mm, 0 for the centred full-fan scans of the
+  configs; a half-fan scan shifts the panel along u)
 The volume is centred at the origin; voxel (i,j,k) is the box
   [ (i-nx/2) hx, (i+1-nx/2) hx ] x [ (j-ny/2) hy, ... ] x [ (k-nz/2) hz, ... ].
 Array layouts: volume f[k][j][i] (x fastest), projections Y[theta][iv][iu] (u fastest).
@@ -32,6 +34,8 @@ class Geometry:
     hx: float = 1.0
     hy: float = 1.0
     hz: float = 1.0
+    off_u: float = 0.0
+    off_v: float = 0.0
 
     def __post_init__(self):
         object.__setattr__(self, "angles", np.ascontiguousarray(self.angles, dtype=np.float64))
@@ -72,8 +76,8 @@ class Geometry:
         """(nv, nu, 3) array of detector pixel centres for angle index ia."""
         t = self.angles[ia]
         c, s = np.cos(t), np.sin(t)
-        uu = (np.arange(self.nu) - (self.nu - 1) / 2.0) * self.du
-        vv = (np.arange(self.nv) - (self.nv - 1) / 2.0) * self.dv
+        uu = (np.arange(self.nu) - (self.nu - 1) / 2.0) * self.du + self.off_u
+        vv = (np.arange(self.nv) - (self.nv - 1) / 2.0) * self.dv + self.off_v
         cen = -(self.sdd - self.sad) * np.array([c, s, 0.0])
         out = np.empty((self.nv, self.nu, 3))
         out[..., 0] = cen[0] + uu[None, :] * (-s)

@@ -26,7 +26,8 @@ class _Geom(C.Structure):
     _fields_ = [("sad", C.c_double), ("sdd", C.c_double), ("n_angles", C.c_int),
                 ("angles", C.POINTER(C.c_double)), ("nu", C.c_int), ("nv", C.c_int),
                 ("du", C.c_double), ("dv", C.c_double), ("nx", C.c_int), ("ny", C.c_int),
-                ("nz", C.c_int), ("hx", C.c_double), ("hy", C.c_double), ("hz", C.c_double)]
+                ("nz", C.c_int), ("hx", C.c_double), ("hy", C.c_double), ("hz", C.c_double),
+                ("off_u", C.c_double), ("off_v", C.c_double)]
 
 
 def lib():
@@ -71,7 +72,7 @@ def _geom(g):
     ang = np.ascontiguousarray(g.angles, dtype=np.float64)
     s = _Geom(float(g.sad), float(g.sdd), int(ang.shape[0]), _dptr(ang), int(g.nu), int(g.nv),
               float(g.du), float(g.dv), int(g.nx), int(g.ny), int(g.nz),
-              float(g.hx), float(g.hy), float(g.hz))
+              float(g.hx), float(g.hy), float(g.hz), float(getattr(g, "off_u", 0.0)), float(getattr(g, "off_v", 0.0)))
     s._keep = ang
     return s
 
@@ -168,5 +169,5 @@ def tv_prox(g, gvol, u0, beta: float, eps: float, omega: float, n_inner: int) ->
 
 from .fbs import (  # noqa: E402  (needs the primitives above)
     energy, fbs_level, fbs_reconstruct, coarsen_geometry, level_geometries,
-    prolong, bin2x2, restrict_volume, lambda_max,
+    prolong, bin2x2, restrict_volume, lambda_max, grad_objective, fbs_vcycle,
 )

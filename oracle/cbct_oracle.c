@@ -41,6 +41,7 @@ typedef struct {
     double du, dv;              /* detector pixel pitch, mm */
     int nx, ny, nz;
     double hx, hy, hz;          /* voxel size, mm */
+    double off_u, off_v;        /* NEXT-3: in-plane shift of the detector panel, mm (0 = centred full-fan, Q14) */
 } og_geom;
 
 int oracle_num_threads(void)
@@ -56,8 +57,8 @@ int oracle_num_threads(void)
 static void ray_endpoints(const og_geom *g, int ia, int iv, int iu, double S[3], double D[3])
 {
     double t = g->angles[ia], c = cos(t), s = sin(t);
-    double uc = ((double)iu - 0.5 * (g->nu - 1)) * g->du;
-    double vc = ((double)iv - 0.5 * (g->nv - 1)) * g->dv;
+    double uc = ((double)iu - 0.5 * (g->nu - 1)) * g->du + g->off_u;
+    double vc = ((double)iv - 0.5 * (g->nv - 1)) * g->dv + g->off_v;
     S[0] = g->sad * c;  S[1] = g->sad * s;  S[2] = 0.0;
     D[0] = -(g->sdd - g->sad) * c + uc * (-s);
     D[1] = -(g->sdd - g->sad) * s + uc * c;
@@ -314,8 +315,8 @@ void oracle_backproject_voxels(const og_geom *g, const double *proj, long n,
                 double P[3] = { (m & 1) ? hi[0] : lo[0], (m & 2) ? hi[1] : lo[1], (m & 4) ? hi[2] : lo[2] };
                 double depth = g->sad - (P[0] * c + P[1] * s);       /* distance from the source along the central ray */
                 double mag = g->sdd / depth;
-                double u = mag * (-P[0] * s + P[1] * c) / g->du + 0.5 * (g->nu - 1);
-                double v = mag * P[2] / g->dv + 0.5 * (g->nv - 1);
+                double u = (mag * (-P[0] * s + P[1] * c) - g->off_u) / g->du + 0.5 * (g->nu - 1);
+                double v = (mag * P[2] - g->off_v) / g->dv + 0.5 * (g->nv - 1);
                 if (u < umin) umin = u;
                 if (u > umax) umax = u;
                 if (v < vmin) vmin = v;
@@ -373,7 +374,7 @@ void oracle_backproject_eq2(const og_geom *g, const double *proj, double *vol)
                 double vstar = (Pt[0] - Cd[0]) * vh[0] + (Pt[1] - Cd[1]) * vh[1] + (Pt[2] - Cd[2]) * vh[2];
                 double l = sqrt(dxs[0] * dxs[0] + dxs[1] * dxs[1] + dxs[2] * dxs[2]);
                 double L = sqrt((Pt[0] - S[0]) * (Pt[0] - S[0]) + (Pt[1] - S[1]) * (Pt[1] - S[1]) + (Pt[2] - S[2]) * (Pt[2] - S[2]));
-                double pu = ustar / g->du + 0.5 * (g->nu - 1), pv = vstar / g->dv + 0.5 * (g->nv - 1);
+                double pu = (ustar - g->off_u) / g->du + 0.5 * (g->nu - 1), pv = (vstar - g->off_v) / g->dv + 0.5 * (g->nv - 1);
                 double fu = floor(pu), fv = floor(pv);
                 int iu = (int)fu, iv = (int)fv;
                 double au = pu - fu, av = pv - fv, val = 0.0;

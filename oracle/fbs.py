@@ -43,8 +43,11 @@ def energy(g, f, Y, mu: float, eps: float, Pf: Optional[np.ndarray] = None) -> d
 def fbs_level(g, Y, f0, n_outer: int, n_inner: int, step: float, mu: float, eps: float,
               omega: float = 1.0, u0_mode: str = "g", clamp: bool = True,
               trace: Optional[list] = None, backprojector: str = "exact",
-              rel_tol: float = 0.0, iters_done: Optional[list] = None) -> np.ndarray:
-    """rel_tol > 0: "Repeat ... until convergence" read as: stop after the first iteration whose update
+              rel_tol: float = 0.0, iters_done: Optional[list] = None, tau: Optional[np.ndarray] = None) -> np.ndarray:
+    """tau (NEXT-3, FAS coarse problems): a linear term -<tau, f> added to the smooth part of the level's objective
+    N_vox E = TV_eps(f) + mu' ||P f - Y||^2, mu' = mu N_vox / (N_theta N_pix); it joins the gradient of step 1:
+    g = f - (1/beta) (2 mu' P^T (P f - Y) - tau) = f - c P^T (P f - Y) + tau / beta.  tau = None is Algorithm A1 as printed.
+    rel_tol > 0: "Repeat ... until convergence" read as: stop after the first iteration whose update
     satisfies ||f_new - f_old||_2 <= rel_tol ||f_new||_2 (NEXT-2; n_outer is then the maximum count);
     the number of iterations run is appended to iters_done.
     backprojector = "exact": dE2/df through the matrix transpose (P:95, the hot path);
@@ -63,6 +66,8 @@ def fbs_level(g, Y, f0, n_outer: int, n_inner: int, step: float, mu: float, eps:
         else:
             G = (g.hx * g.hy * g.hz / (g.du * g.dv)) * o.backproject_eq2(g, r)   # eq. 2
         gv = f - c * G                               # step 1
+        if tau is not None:
+            gv = gv + tau / beta                     # FAS right-hand side (Q21)
         u0 = gv if u0_mode == "g" else f             # Q7: start of the inner descent
         u = o.tv_prox(g, gv, u0, beta, eps, omega, n_inner)   # step 2
         f = np.maximum(u, 0.0) if clamp else u       # step 3             (Q18)
@@ -86,9 +91,10 @@ def coarsen_axes(g) -> tuple:
     return tuple(ha <= math.sqrt(2.0) * m * (1.0 + 1e-9) for ha in h)
 
 
-def coarsen_geometry(g):
+def coarsen_geometry(g, bin_detector: bool = True):
     """Next-coarser level: halve the dims / double the spacing on coarsen_axes; bin the detector
-    2x2 (pitch doubles) iff both x and y were coarsened.  Returns (geometry, axes, binned)."""
+    2x2 (pitch doubles) iff both x and y were coarsened.  Returns (geometry, axes, binned).
+    bin_detector = False (NEXT-3, Q20): the coarse levels keep the detector, and the data, at full resolution."""
     ax = coarsen_axes(g)
     n = [g.nx, g.ny, g.nz]
     h = [g.hx, g.hy, g.hz]
@@ -98,7 +104,7 @@ def coarsen_geometry(g):
                 raise ValueError("odd dimension on an axis that must coarsen")
             n[a] //= 2
             h[a] *= 2.0
-    binned = bool(ax[0] and ax[1])
+    binned = bool(ax[0] and ax[1]) and bin_detector
     nu, nv, du, dv = g.nu, g.nv, g.du, g.dv
     if binned:
         if nu % 2 or nv % 2:
@@ -108,11 +114,11 @@ def coarsen_geometry(g):
     return gc, ax, binned
 
 
-def level_geometries(g, n_levels: int):
+def level_geometries(g, n_levels: int, bin_detector: bool = True):
     """[level 0 (finest), ..., level n_levels-1 (coarsest)] with the transfer descriptors."""
     geoms, axes, binned = [g], [], []
     for _ in range(n_levels - 1):
-        gc, ax, b = coarsen_geometry(geoms[-1])
+        gc, ax, b = coarsen_geometry(geoms[-1], bin_detector)
         geoms.append(gc)
         axes.append(ax)
         binned.append(b)
@@ -162,12 +168,12 @@ def prolong(c: np.ndarray, axes) -> np.ndarray:
 def fbs_reconstruct(g, Y, f0, n_levels: int, n_outer: Sequence[int], n_inner: int, step: float,
                     mu: float, eps: float, omega: float = 1.0, u0_mode: str = "g",
                     clamp: bool = True, trace: Optional[list] = None, backprojector: str = "exact",
-                    rel_tol: float = 0.0, iters_done: Optional[list] = None) -> np.ndarray:
+                    rel_tol: float = 0.0, iters_done: Optional[list] = None, bin_detector: bool = True) -> np.ndarray:
     """O6: run O5 at the coarsest level from f0 (zeros if None; a caller's fine-grid f0 is
     restricted down), prolong to the next level, repeat; n_outer is listed coarsest first.
     n_levels = 1 is exactly O5."""
     assert len(n_outer) == n_levels
-    geoms, axes, binned = level_geometries(g, n_levels)
+    geoms, axes, binned = level_geometries(g, n_levels, bin_detector)
     Ys = [np.asarray(Y, dtype=np.float64)]
     for b in binned:
         Ys.append(bin2x2(Ys[-1]) if b else Ys[-1])
@@ -183,6 +189,65 @@ def fbs_reconstruct(g, Y, f0, n_levels: int, n_outer: Sequence[int], n_inner: in
                       rel_tol=rel_tol, iters_done=iters_done)
         if lev > 0:
             f = prolong(f, axes[lev - 1])
+    return f
+
+
+# ----------------------------------------------------------------------------------------
+# NEXT-3: FAS V-cycles ("multi-grid method", ref. 20 = Brandt; no details given: reading Q21)
+#
+# Every level l has the same kind of objective, scaled by its voxel count:
+#   F_l(f) = N_vox,l E_eps,l(f) = TV_eps,l(f) + mu'_l ||P_l f - Y_l||^2,  mu'_l = mu N_vox,l / (N_theta N_pix,l),
+# whose gradient  grad F_l(f) = grad TV_eps,l(f) + 2 mu'_l P_l^T (P_l f - Y_l)  is a discretisation of the
+# level-independent functional derivative V dE/df (P:65-69 normalise E1 by V and E2 by A), so gradients can be moved
+# between levels by plain averaging.  Brandt's full approximation scheme for the nonlinear problem:
+#   V(l, f, tau):   f <- nu_pre iterations of A1 on  F_l(f) - <tau, f>                      (pre-smoothing)
+#                   if l is not the coarsest level:
+#                       f_H0  = R f                     (R = mean of the children, restrict_volume)
+#                       tau_H = grad F_{l+1}(f_H0) - R (grad F_l(f) - tau)                 (residual restriction)
+#                       f_H   = V(l+1, f_H0, tau_H)
+#                       f <- max(f + Prolong(f_H - f_H0), 0)                                (correction, kept feasible: P:91)
+#                       f <- nu_post iterations of A1 on  F_l(f) - <tau, f>                 (post-smoothing)
+#   at the coarsest level the smoother runs nu_coarse iterations instead.
+# The finest level has tau = 0.  The linear term enters A1 through step 1 (fbs_level(tau=...)).
+# ----------------------------------------------------------------------------------------
+def grad_objective(g, f, Y, mu: float, eps: float) -> np.ndarray:
+    """grad F_l(f) = grad TV_eps(f) + 2 mu' P^T (P f - Y),  mu' = mu N_vox / (N_theta N_pix)   (N_vox times the gradient of O3)."""
+    o = _prims()
+    mu_p = mu * g.n_vox / (g.n_angles * g.n_pix)
+    return o.tv_grad(g, f, eps) + 2.0 * mu_p * o.backproject(g, o.forward(g, f) - Y)
+
+
+def fbs_vcycle(g, Y, f0, n_levels: int, n_cycles: int, nu_pre: int, nu_post: int, nu_coarse: int, n_inner: int,
+               step: float, mu: float, eps: float, omega: float = 1.0, bin_detector: bool = True,
+               trace: Optional[list] = None) -> np.ndarray:
+    """n_cycles FAS V-cycles on the finest level, starting from f0 (zeros if None).  n_levels = 1 is plain A1 with
+    n_cycles * nu_coarse iterations.  trace (optional) receives energy(f) after every cycle."""
+    geoms, axes, binned = level_geometries(g, n_levels, bin_detector)
+    Ys = [np.asarray(Y, dtype=np.float64)]
+    for b in binned:
+        Ys.append(bin2x2(Ys[-1]) if b else Ys[-1])
+
+    def smooth(l, f, tau, n):
+        return fbs_level(geoms[l], Ys[l], f, n, n_inner, step, mu, eps, omega, tau=tau)
+
+    def V(l, f, tau):
+        if l == n_levels - 1:
+            return smooth(l, f, tau, nu_coarse)
+        f = smooth(l, f, tau, nu_pre)
+        D = grad_objective(geoms[l], f, Ys[l], mu, eps)
+        if tau is not None:
+            D = D - tau
+        fH0 = restrict_volume(f, axes[l])
+        tauH = grad_objective(geoms[l + 1], fH0, Ys[l + 1], mu, eps) - restrict_volume(D, axes[l])
+        fH = V(l + 1, fH0, tauH)
+        f = np.maximum(f + prolong(fH - fH0, axes[l]), 0.0)
+        return smooth(l, f, tau, nu_post)
+
+    f = np.zeros(g.vol_shape) if f0 is None else np.array(f0, dtype=np.float64, copy=True)
+    for _ in range(n_cycles):
+        f = V(0, f, None)
+        if trace is not None:
+            trace.append(energy(g, f, Ys[0], mu, eps))
     return f
 
 

@@ -73,6 +73,10 @@ __global__ void __launch_bounds__(128) prefix_kernel(const DevGeom d, const floa
 }
 
 
+#ifndef CBCT_BP_VOTE
+#define CBCT_BP_VOTE 1
+#endif
+
 template <int KC, int BI>
 __global__ void __launch_bounds__(32 * BI)
 backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restrict__ angle_has,
@@ -154,25 +158,30 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
                         vTn = min(max(vTn, 0), d.nv);
                     }
                     const float2 c2 = __ldg(C + (offC + vT * d.nu));
-                    // rays crossing plane k0+q inside the slab: v in [min(vT,vTn), max(vT,vTn)).  The arithmetic of the first
-                    // one runs unconditionally (its y is 0 if there is none).
+                    // rays crossing plane k0+q inside the slab: v in [min(vT,vTn), max(vT,vTn)) (y = 0 stands in if there is none).
                     // b = lambda at which the ray meets the plane: T(lambda) zeta(v) = zk with T(lambda) = T + lambda dt and
                     // zeta(v) = (v - cv) dv / hz, i.e. b = (zk - T zeta(v)) / (dt zeta(v)), the projector's b with its numerator
                     // taken by one FMA (a ray in the central plane, v = cv, crosses nothing; saturation turns its 0/0 into 0).
-                    const int dlt = vTn - vT, vs = min(vT, vTn);
-                    const float vf = (float)vs - cv;
-                    const float bq = __saturatef(fmaf(-Tdv, vf, zk) * rcp_approx(vf * dtdv));
-                    // rising iff dt zeta(v) > 0: move the sign bit of dt zeta(v) onto y
-                    float yq = 0.f;
-                    if (dlt != 0) yq = __ldg(rs + (offR + vs * d.nu));
-                    yq = __int_as_float(__float_as_int(yq) ^ (__float_as_int(vf * dtdv) & 0x80000000));
-                    float up = fmaxf(0.f, l1 - fmaxf(l0, bq)) * yq;   // moved up across the plane (negative: moved down)
-                    if constexpr (MULTI) {
-                        for (int v = vs + 1; v < vs + abs(dlt); ++v) {   // further rays crossing this plane (fine detector rows)
-                            const float vf2 = (float)v - cv;
-                            const float b2 = __saturatef(fmaf(-Tdv, vf2, zk) * rcp_approx(vf2 * dtdv));
-                            const float y2 = __ldg(rs + (offR + v * d.nu));
-                            up = fmaf(fmaxf(0.f, l1 - fmaxf(l0, b2)), __int_as_float(__float_as_int(y2) ^ (__float_as_int(vf * dtdv) & 0x80000000)), up);
+                    // Only ~5 % of the (lane, plane) pairs have such a ray.  The lanes of a warp are adjacent minor rows of ONE
+                    // slab, so their ray depths T and with them their bounds are nearly equal and the crossings cluster: the warp
+                    // skips the crossing arithmetic (17 of the 31 instructions of a plane) when none of its converged lanes has one.
+                    float up = 0.f;                    // moved up across the plane (negative: moved down)
+                    if (!CBCT_BP_VOTE || __any_sync(__activemask(), vT != vTn)) {
+                        const int dlt = vTn - vT, vs = min(vT, vTn);
+                        const float vf = (float)vs - cv;
+                        const float bq = __saturatef(fmaf(-Tdv, vf, zk) * rcp_approx(vf * dtdv));
+                        // rising iff dt zeta(v) > 0: move the sign bit of dt zeta(v) onto y
+                        float yq = 0.f;
+                        if (dlt != 0) yq = __ldg(rs + (offR + vs * d.nu));
+                        yq = __int_as_float(__float_as_int(yq) ^ (__float_as_int(vf * dtdv) & 0x80000000));
+                        up = fmaxf(0.f, l1 - fmaxf(l0, bq)) * yq;
+                        if constexpr (MULTI) {
+                            for (int v = vs + 1; v < vs + abs(dlt); ++v) {   // further rays crossing this plane (fine detector rows)
+                                const float vf2 = (float)v - cv;
+                                const float b2 = __saturatef(fmaf(-Tdv, vf2, zk) * rcp_approx(vf2 * dtdv));
+                                const float y2 = __ldg(rs + (offR + v * d.nu));
+                                up = fmaf(fmaxf(0.f, l1 - fmaxf(l0, b2)), __int_as_float(__float_as_int(y2) ^ (__float_as_int(vf * dtdv) & 0x80000000)), up);
+                            }
                         }
                     }
                     if (q > 0) {

@@ -14,8 +14,9 @@ def ray_endpoints(g):
     t = np.asarray(g.angles)
     c, s = np.cos(t), np.sin(t)
     S = np.stack([g.sad * c, g.sad * s, np.zeros_like(t)], axis=-1)
-    uu = (np.arange(g.nu) - (g.nu - 1) / 2.0) * g.du
-    vv = (np.arange(g.nv) - (g.nv - 1) / 2.0) * g.dv
+    # a shifted panel (half-fan): every pixel centre moves by (off_u, off_v) in the detector plane
+    uu = np.linspace(-(g.nu - 1) / 2.0, (g.nu - 1) / 2.0, g.nu) * g.du + getattr(g, "off_u", 0.0)
+    vv = np.linspace(-(g.nv - 1) / 2.0, (g.nv - 1) / 2.0, g.nv) * g.dv + getattr(g, "off_v", 0.0)
     D = np.empty((len(t), g.nv, g.nu, 3))
     D[..., 0] = (-(g.sdd - g.sad) * c)[:, None, None] + uu[None, None, :] * (-s)[:, None, None]
     D[..., 1] = (-(g.sdd - g.sad) * s)[:, None, None] + uu[None, None, :] * c[:, None, None]
@@ -139,10 +140,83 @@ def eq2_backproject(g, r):
         c, s = np.cos(th), np.sin(th)
         t = g.sad - (X * c + Y * s)
         lat = -X * s + Y * c
-        pu = g.sdd * lat / t / g.du + (g.nu - 1) / 2.0
-        pv = g.sdd * Z / t / g.dv + (g.nv - 1) / 2.0
+        pu = (g.sdd * lat / t - getattr(g, "off_u", 0.0)) / g.du + (g.nu - 1) / 2.0
+        pv = (g.sdd * Z / t - getattr(g, "off_v", 0.0)) / g.dv + (g.nv - 1) / 2.0
         val = map_coordinates(np.asarray(r[ia], dtype=np.float64), [pv.ravel(), pu.ravel()], order=1,
                               mode="grid-constant", cval=0.0).reshape(g.vol_shape)
         w = (g.sdd / t) ** 2 * np.sqrt(t * t + lat * lat + Z * Z) / t
         out += w * val
     return out
+
+
+# ------------------------------------------------ NEXT-3: FAS V-cycle with explicit matrices -----
+def _axis_restrict(n_fine):
+    """(n_fine/2, n_fine): mean of the two children."""
+    R = np.zeros((n_fine // 2, n_fine))
+    for I in range(n_fine // 2):
+        R[I, 2 * I] = 0.5
+        R[I, 2 * I + 1] = 0.5
+    return R
+
+
+def _axis_prolong(n_coarse):
+    """(2 n_coarse, n_coarse): fine 2I = 3/4 c[I] + 1/4 c[I-1], fine 2I+1 = 3/4 c[I] + 1/4 c[I+1], indices clamped."""
+    P = np.zeros((2 * n_coarse, n_coarse))
+    for I in range(n_coarse):
+        P[2 * I, I] += 0.75
+        P[2 * I, max(I - 1, 0)] += 0.25
+        P[2 * I + 1, I] += 0.75
+        P[2 * I + 1, min(I + 1, n_coarse - 1)] += 0.25
+    return P
+
+
+def transfer_matrices(g_fine, g_coarse):
+    """Dense restriction (n_c x n_f) and prolongation (n_f x n_c) between two levels, volumes flattened [k][j][i];
+    an axis that keeps its size gets the identity."""
+    def ax(nf, nc):
+        return (np.eye(nf), np.eye(nf)) if nf == nc else (_axis_restrict(nf), _axis_prolong(nc))
+    Rx, Px = ax(g_fine.nx, g_coarse.nx)
+    Ry, Py = ax(g_fine.ny, g_coarse.ny)
+    Rz, Pz = ax(g_fine.nz, g_coarse.nz)
+    return np.kron(Rz, np.kron(Ry, Rx)), np.kron(Pz, np.kron(Py, Px))
+
+
+def dense_vcycle(levels, f0, n_cycles, nu_pre, nu_post, nu_coarse, n_inner, step, mu, eps, omega=1.0):
+    """Brandt's full approximation scheme around Algorithm A1, written with explicit matrices.
+    levels[l] = dict(g=geometry, A=dense system matrix, Y=data); level 0 is the finest.  Objective per level
+    F(f) = TV_eps(f) + mu' |A f - y|^2 with mu' = mu N_vox/(N_theta N_pix); smoother = A1 with the extra gradient term -tau."""
+    beta = mu / step
+    T = [transfer_matrices(levels[l]["g"], levels[l + 1]["g"]) for l in range(len(levels) - 1)]
+
+    def grad(l, f):
+        g, A, y = levels[l]["g"], levels[l]["A"], levels[l]["Y"].ravel()
+        mu_p = mu * g.n_vox / (g.n_angles * g.n_pix)
+        return tv_grad(f.reshape(g.vol_shape), g, eps).ravel() + 2.0 * mu_p * (A.T @ (A @ f - y))
+
+    def smooth(l, f, tau, n):
+        g, A, y = levels[l]["g"], levels[l]["A"], levels[l]["Y"].ravel()
+        c = 2.0 * step * g.n_vox / (g.n_angles * g.n_pix)
+        dt = omega / (beta + 4.0 * (1 / g.hx ** 2 + 1 / g.hy ** 2 + 1 / g.hz ** 2) / eps)
+        for _ in range(n):
+            gv = f - c * (A.T @ (A @ f - y)) + tau / beta
+            u = gv.copy()
+            for _ in range(n_inner):
+                u = u - dt * (beta * (u - gv) + tv_grad(u.reshape(g.vol_shape), g, eps).ravel())
+            f = np.maximum(u, 0.0)
+        return f
+
+    def V(l, f, tau):
+        if l == len(levels) - 1:
+            return smooth(l, f, tau, nu_coarse)
+        f = smooth(l, f, tau, nu_pre)
+        R, P = T[l]
+        fH0 = R @ f
+        tauH = grad(l + 1, fH0) - R @ (grad(l, f) - tau)
+        fH = V(l + 1, fH0, tauH)
+        f = np.maximum(f + P @ (fH - fH0), 0.0)
+        return smooth(l, f, tau, nu_post)
+
+    f = f0.ravel().astype(np.float64).copy()
+    for _ in range(n_cycles):
+        f = V(0, f, np.zeros_like(f))
+    return f.reshape(levels[0]["g"].vol_shape)
