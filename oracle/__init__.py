@@ -7,6 +7,7 @@ Layout:
   cbct_oracle.c   O1 projector (Siddon merge), O2 literal-scatter transpose, brute-force
                   per-voxel clipping, O3/O4 smoothed TV value / gradient / inner descent  (C, OpenMP)
   fbs.py          O3 energy, O5 outer FBS loop, O6 multigrid cascade and its transfers      (numpy)
+  fdk.py          NEXT-4: the FDK baseline (cosine pre-weight, ramp filter, weighted backprojection)    (numpy + C)
   build.py        gcc build of liboracle.so (also run by __graft_entry__.build())
 See each function's docstring for the PAPER.md passage it follows.
 """
@@ -47,6 +48,8 @@ def lib():
         L.oracle_backproject_voxels.argtypes = [gp, dp, C.c_long, ip, ip, ip, dp]
         L.oracle_backproject_eq2.argtypes = [gp, dp, dp]
         L.oracle_backproject_eq2.restype = None
+        L.oracle_fdk_backproject.argtypes = [gp, dp, C.c_double, dp]
+        L.oracle_fdk_backproject.restype = None
         d, i = C.c_double, C.c_int
         L.oracle_tv_value.argtypes = [dp, i, i, i, d, d, d, d]
         L.oracle_tv_value.restype = d
@@ -143,6 +146,15 @@ def backproject_eq2(g, proj) -> np.ndarray:
     return out
 
 
+def fdk_backproject(g, q, scale: float) -> np.ndarray:
+    """FDK backprojection step: scale * sum_theta SAD^2/U^2 q(u*,v*) (see oracle/fdk.py for the whole algorithm)."""
+    q = _proj(g, q)
+    out = np.empty(g.vol_shape)
+    gs = _geom(g)
+    lib().oracle_fdk_backproject(C.byref(gs), _dptr(q), float(scale), _dptr(out))
+    return out
+
+
 def tv_value(g, f, eps: float) -> float:
     """O3: TV_eps(f) = sum_ijk sqrt(dx^2+dy^2+dz^2+eps^2)  (PAPER.md:69 E1 times N_vox; eps=0 is the paper's)."""
     f = _vol(g, f)
@@ -171,3 +183,4 @@ from .fbs import (  # noqa: E402  (needs the primitives above)
     energy, fbs_level, fbs_reconstruct, coarsen_geometry, level_geometries,
     prolong, bin2x2, restrict_volume, lambda_max, grad_objective, fbs_vcycle,
 )
+from .fdk import fdk_reconstruct, fdk_preweight, fdk_ramp_kernel, fdk_filter  # noqa: E402

@@ -392,6 +392,48 @@ void oracle_backproject_eq2(const og_geom *g, const double *proj, double *vol)
     }
 }
 
+/*
+ * NEXT-4: the backprojection step of the FDK algorithm (Feldkamp, Davis, Kress; ref. 1 of the paper; the paper's
+ * comparison images Fig. 1(d), Fig. 2 at P:105, P:125 are FDK reconstructions):
+ *   f(x) = (dtheta / 2) sum_theta  SAD^2 / U^2(x, theta)  q^theta(u*, v*),
+ * q the pre-weighted, ramp-filtered projections (oracle/fdk.py), x the voxel centre, U = SAD - (x cos theta + y sin theta)
+ * the distance of x from the source along the central ray, (u*,v*) = SDD (lat, z) / U the point where the line
+ * source -> x meets the imager; q at (u*,v*) bilinear between pixel centres, 0 outside the detector (as Q4).
+ * `scale` = dtheta / 2 is passed in (equally spaced full rotation: dtheta = 2 pi / N_theta).
+ */
+void oracle_fdk_backproject(const og_geom *g, const double *q, double scale, double *vol)
+{
+#pragma omp parallel for schedule(static)
+    for (long kj = 0; kj < (long)g->nz * g->ny; ++kj) {
+        int k = (int)(kj / g->ny), j = (int)(kj % g->ny);
+        for (int i = 0; i < g->nx; ++i) {
+            double x = ((double)i - 0.5 * (g->nx - 1)) * g->hx, y = ((double)j - 0.5 * (g->ny - 1)) * g->hy,
+                   z = ((double)k - 0.5 * (g->nz - 1)) * g->hz;
+            double acc = 0.0;
+            for (int ia = 0; ia < g->n_angles; ++ia) {
+                double t = g->angles[ia], c = cos(t), s = sin(t);
+                double U = g->sad - (x * c + y * s);
+                if (U <= 0.0) continue;
+                double lat = -x * s + y * c;
+                double ustar = g->sdd * lat / U, vstar = g->sdd * z / U;
+                double pu = (ustar - g->off_u) / g->du + 0.5 * (g->nu - 1), pv = (vstar - g->off_v) / g->dv + 0.5 * (g->nv - 1);
+                double fu = floor(pu), fv = floor(pv);
+                int iu = (int)fu, iv = (int)fv;
+                double au = pu - fu, av = pv - fv, val = 0.0;
+                const double *img = q + (size_t)ia * g->nv * g->nu;
+                for (int dv_ = 0; dv_ < 2; ++dv_)
+                    for (int du_ = 0; du_ < 2; ++du_) {
+                        int uu = iu + du_, vv = iv + dv_;
+                        if (uu < 0 || uu >= g->nu || vv < 0 || vv >= g->nv) continue;
+                        val += (du_ ? au : 1.0 - au) * (dv_ ? av : 1.0 - av) * img[(size_t)vv * g->nu + uu];
+                    }
+                acc += (g->sad * g->sad) / (U * U) * val;
+            }
+            vol[((size_t)k * g->ny + j) * g->nx + i] = scale * acc;
+        }
+    }
+}
+
 /* ------------------------------------------------------------------------------------
  * O3 / O4: smoothed isotropic total variation (P:69 E1, ROF semi-norm of ref. 5; Q5, Q6).
  *   d_x = (f[i+1]-f[i])/hx  (0 at the last index: Neumann), likewise d_y, d_z

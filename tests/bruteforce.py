@@ -220,3 +220,24 @@ def dense_vcycle(levels, f0, n_cycles, nu_pre, nu_post, nu_coarse, n_inner, step
     for _ in range(n_cycles):
         f = V(0, f, np.zeros_like(f))
     return f.reshape(levels[0]["g"].vol_shape)
+
+
+# ------------------------------------------------ NEXT-4: FDK backprojection a second time -----
+def fdk_backproject(g, q, scale):
+    """scale * sum_theta SAD^2/U^2 q(u*,v*), the interpolation done by scipy.ndimage.map_coordinates (order 1, zero beyond
+    the grid), coordinates from similar triangles."""
+    from scipy.ndimage import map_coordinates
+    xs = (np.arange(g.nx) - (g.nx - 1) / 2.0) * g.hx
+    ys = (np.arange(g.ny) - (g.ny - 1) / 2.0) * g.hy
+    zs = (np.arange(g.nz) - (g.nz - 1) / 2.0) * g.hz
+    Z, Y, X = np.meshgrid(zs, ys, xs, indexing="ij")
+    out = np.zeros(g.vol_shape)
+    for ia, th in enumerate(np.asarray(g.angles)):
+        c, s = np.cos(th), np.sin(th)
+        U = g.sad - (X * c + Y * s)
+        pu = (g.sdd * (-X * s + Y * c) / U - getattr(g, "off_u", 0.0)) / g.du + (g.nu - 1) / 2.0
+        pv = (g.sdd * Z / U - getattr(g, "off_v", 0.0)) / g.dv + (g.nv - 1) / 2.0
+        val = map_coordinates(np.asarray(q[ia], dtype=np.float64), [pv.ravel(), pu.ravel()], order=1,
+                              mode="grid-constant", cval=0.0).reshape(g.vol_shape)
+        out += (g.sad / U) ** 2 * val
+    return scale * out
