@@ -317,7 +317,7 @@ def run_sharded(args):
     the ranks and one NCCL all-reduce of the gradient volume per outer iteration; strong scaling."""
     import torch
     import paper_1002_3675_b200 as cb
-    from paper_1002_3675_b200.sharded import CudaOps, fbs_reconstruct_sharded, shard_angles
+    from paper_1002_3675_b200.sharded import fbs_reconstruct_sharded, shard_angles
     from cbct_synth import make_config
     rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -333,12 +333,11 @@ def run_sharded(args):
     mine = shard_angles(g.n_angles, rank, world)
     G = cb.Geometry.from_synth(g.with_angles(g.angles[mine]))
     d_Y = torch.from_numpy(np.ascontiguousarray(cfg.projections(mine), dtype=np.float32)).to(dev)
-    ops = CudaOps(G, LEVELS)
     state = {"f": torch.zeros(g.vol_shape, device=dev)}
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
 
     def step():
-        state["f"] = fbs_reconstruct_sharded(ops, d_Y, state["f"], LEVELS, [1] * LEVELS, N_INNER, cfg.step, cfg.mu, cfg.eps,
+        state["f"] = fbs_reconstruct_sharded(G, d_Y, state["f"], LEVELS, [1] * LEVELS, N_INNER, cfg.step, cfg.mu, cfg.eps,
                                              cfg.omega, g.n_angles, dist)
 
     for _ in range(args.warmup):

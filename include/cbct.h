@@ -65,6 +65,19 @@ cbct_status cbct_geometry_create(double sad_mm, double sdd_mm,
                                  int nx, int ny, int nz, double hx_mm, double hy_mm, double hz_mm,
                                  cbct_geometry **out);
 
+/*
+ * NEXT-3 (reading Q19): the same with the detector panel shifted in its own plane by (off_u_mm, off_v_mm): pixel (iu,iv)
+ * sits at ((iu-(nu-1)/2) du + off_u, (iv-(nv-1)/2) dv + off_v) about the point where the central ray meets the imager
+ * (half-fan scans shift the panel along u; the paper's scans are centred full-fan).  Source, central ray and L0 = sdd
+ * are unchanged; coarse levels keep the shift.  Zero offsets give exactly cbct_geometry_create.  Errors as there, plus
+ * INVALID_ARG for a non-finite offset.
+ */
+cbct_status cbct_geometry_create_ex(double sad_mm, double sdd_mm,
+                                    const double *h_angles_rad, int n_angles,
+                                    int nu, int nv, double du_mm, double dv_mm, double off_u_mm, double off_v_mm,
+                                    int nx, int ny, int nz, double hx_mm, double hy_mm, double hz_mm,
+                                    cbct_geometry **out);
+
 /* Frees the handle, its coarse-level handles and all scratch.  NULL is allowed.  Synchronises the device. */
 void cbct_geometry_destroy(cbct_geometry *g);
 
@@ -80,6 +93,13 @@ cbct_status cbct_geometry_query(const cbct_geometry *g, int *h_dims6, double *h_
  * Errors: SHAPE for an odd dimension on an axis that must coarsen (or odd nu/nv when binning).
  */
 cbct_status cbct_geometry_coarsen(const cbct_geometry *g, cbct_geometry **out_coarse, int *h_flags4);
+
+/*
+ * NEXT-3 (reading Q20): whether the coarse multigrid levels bin the detector 2x2 (on = 1, the default, O6) or keep the
+ * detector and the data at full resolution (on = 0).  Changing the choice drops the handle's existing coarse levels
+ * (synchronises the device); they are rebuilt on demand.  Applies to every cascade / V-cycle run on this handle.
+ */
+cbct_status cbct_set_detector_binning(cbct_geometry *g, int on);
 
 /*
  * a1. Forward projection q = P f (definition O1): for every angle and detector pixel,
@@ -186,6 +206,34 @@ cbct_status cbct_fbs_reconstruct_until(const cbct_geometry *g, const float *d_Y,
                                        float *d_f_out, int *h_iters_per_level, void *cuda_stream);
 
 /*
+ * NEXT-3 (reading Q21). FAS V-cycles around Algorithm A1 ("multi-grid method", ref. 20 at P:170 is Brandt; the paper
+ * gives no details).  Level l carries F_l(f) = TV_eps(f) + mu'_l ||P_l f - Y_l||^2, mu'_l = mu N_vox,l / (N_theta N_pix,l)
+ * (= N_vox,l times the energy of eq. 1).  One cycle on level l with right-hand side tau (0 on the finest level):
+ *     nu_pre iterations of A1 on F_l - <tau, .>   (step 1 becomes gv = f - c G + tau / beta)
+ *     f_H0 = R f;  tau_H = grad F_{l+1}(f_H0) - R (grad F_l(f) - tau);  f_H = cycle(l+1, f_H0, tau_H)
+ *     f = max(f + Prolong(f_H - f_H0), 0);  nu_post iterations of A1 on F_l - <tau, .>
+ * and nu_coarse iterations at the coarsest level.  R = mean of the children (cbct_restrict), Prolong = cbct_prolong,
+ * Y on the coarse levels as in cbct_fbs_reconstruct.  n_cycles cycles start from d_f0 (NULL = zeros); n_levels == 1 is
+ * n_cycles * nu_coarse iterations of plain A1.  d_f_out (finest level) may equal d_f0.
+ * h_energy_trace: NULL or n_cycles doubles receiving E_eps after every cycle (synchronises per cycle).
+ * Errors: INVALID_ARG for n_levels < 1, negative counts, step/mu/eps/omega <= 0; SHAPE as for cbct_geometry_coarsen.
+ */
+cbct_status cbct_fbs_vcycle(const cbct_geometry *g, const float *d_Y, const float *d_f0,
+                            int n_levels, int n_cycles, int nu_pre, int nu_post, int nu_coarse, int n_tv_inner,
+                            float step, float mu, float eps, float omega,
+                            float *d_f_out, double *h_energy_trace, void *cuda_stream);
+
+/*
+ * NEXT-4. The FDK reconstruction the paper compares against (Feldkamp-Davis-Kress, ref. 1 at P:147; Fig. 1(d) P:105,
+ * Fig. 2), reading Q22: d_vol = (pi/N_theta) sum_theta SAD^2/U^2 q_theta(u*,v*) with q the cosine-weighted
+ * (SDD/sqrt(SDD^2+u^2+v^2)) projections filtered along u by the band-limited ramp kernel at pitch du SAD/SDD, U the distance
+ * of the voxel from the source along the central ray, bilinear interpolation, zero outside the detector.  Valid for equally
+ * spaced views over a full rotation (no short-scan or half-fan redundancy weights, no apodisation).  d_vol is overwritten.
+ * Errors: SHAPE if nu > 17066 (the filter keeps a zero-padded row in shared memory).
+ */
+cbct_status cbct_fdk_reconstruct(const cbct_geometry *g, const float *d_Y, float *d_vol, void *cuda_stream);
+
+/*
  * NEXT-4. The two halves of one outer iteration of A1, for drivers that put an exchange step between them: with
  * the angle list partitioned over several GPUs (one handle per GPU holding its share of the angles and of d_Y),
  * every GPU computes its partial data gradient, the partial volumes are summed (one all-reduce), and every GPU
@@ -199,6 +247,52 @@ cbct_status cbct_fbs_reconstruct_until(const cbct_geometry *g, const float *d_Y,
 cbct_status cbct_data_gradient(const cbct_geometry *g, const float *d_f, const float *d_Y, float *d_G, void *cuda_stream);
 cbct_status cbct_prox_step(const cbct_geometry *g, const float *d_f, const float *d_G, float c, float beta,
                            float eps, float omega, int n_inner, float *d_f_out, void *cuda_stream);
+
+/*
+ * NEXT-4. The angle-sharded cascade itself: this handle holds THIS RANK'S share of the views and d_Y_local
+ * their data; every rank holds the whole volume.  Per outer iteration: cbct_data_gradient -> `allreduce` (sum of the gradient
+ * volume over the ranks, in place) -> cbct_prox_step with c = 2 step N_vox / (n_angles_total N_pix), inside the same
+ * coarse-to-fine cascade as cbct_fbs_reconstruct (n_outer_per_level COARSEST FIRST, d_f0 NULL = zeros).
+ *   allreduce(d_buf, count, user, cuda_stream): must sum d_buf[0..count) over all ranks in place, ordered on cuda_stream
+ *     (e.g. ncclAllReduce, or torch.distributed.all_reduce on the tensor that owns d_buf); returns 0 on success.
+ *     NULL = single rank (the result then equals cbct_fbs_reconstruct).
+ *   d_G_scratch: caller-owned device buffer of nx*ny*nz floats — the buffer handed to `allreduce` (its first N_vox,l floats
+ *     on level l), so the caller knows which of its tensors is exchanged.  Must not alias d_f_out.
+ * Errors: INVALID_ARG (NULL, bad counts, n_angles_total < this handle's views, callback failure), SHAPE as for coarsen.
+ */
+typedef int (*cbct_allreduce_fn)(float *d_buf, unsigned long long count, void *user, void *cuda_stream);
+cbct_status cbct_fbs_reconstruct_sharded(const cbct_geometry *g, const float *d_Y_local, const float *d_f0,
+                                         int n_levels, const int *n_outer_per_level, int n_tv_inner,
+                                         float step, float mu, float eps, float omega, int n_angles_total,
+                                         cbct_allreduce_fn allreduce, void *user, float *d_G_scratch,
+                                         float *d_f_out, void *cuda_stream);
+
+/*
+ * The order of operations of that cascade, as a routine over callbacks (host logic only, makes no CUDA call): used by
+ * cbct_fbs_reconstruct_sharded with this library's operators, and callable with any other operators that keep the
+ * per-level state themselves (the CPU multi-rank tests drive it with the fp64 oracle over gloo).  Every callback returns
+ * 0 on success (a cbct_status value is passed through).  Levels: 0 = finest ... n_levels-1 = coarsest.
+ *   level_sizes(user, l, &n_vox, &n_pix)   sizes of level l (n_pix = nu*nv of that level)
+ *   bin(user, l)                           Y_{l+1} = 2x2-binned Y_l
+ *   start(user, L, have_f0)                f_L = 0, or the caller's f0 restricted level by level down to L
+ *   data_gradient(user, l)                 G_l = P^T (P f_l - Y_l) over this rank's views
+ *   all_reduce(user, l)                    G_l summed over the ranks (may be NULL: single rank)
+ *   prox_step(user, l, c, beta)            f_l = max(0, TVprox(f_l - c G_l))
+ *   prolong(user, l)                       f_{l-1} = Prolong f_l
+ * with c = 2 step N_vox,l / (n_angles_total N_pix,l) and beta = mu / step.
+ */
+typedef struct cbct_cascade_ops {
+    void *user;
+    int (*level_sizes)(void *user, int level, unsigned long long *n_vox, unsigned long long *n_pix);
+    int (*bin)(void *user, int level);
+    int (*start)(void *user, int coarsest_level, int have_f0);
+    int (*data_gradient)(void *user, int level);
+    int (*all_reduce)(void *user, int level);
+    int (*prox_step)(void *user, int level, double c, double beta);
+    int (*prolong)(void *user, int level);
+} cbct_cascade_ops;
+cbct_status cbct_cascade_run(const cbct_cascade_ops *ops, int n_levels, const int *n_outer_per_level,
+                             double step, double mu, int n_angles_total, int have_f0);
 
 /*
  * Host-buffer variants (end-to-end path): same operations with HOST pointers; each call copies its

@@ -14,11 +14,26 @@ STATUS = {0: "CBCT_OK", 1: "CBCT_ERR_INVALID_ARG", 2: "CBCT_ERR_SHAPE", 3: "CBCT
 
 # every symbol include/cbct.h declares (tests check that the library exports each of them)
 SYMBOLS = (
-    "cbct_geometry_create", "cbct_geometry_destroy", "cbct_geometry_query", "cbct_geometry_coarsen",
+    "cbct_geometry_create", "cbct_geometry_create_ex", "cbct_set_detector_binning", "cbct_fbs_vcycle", "cbct_fdk_reconstruct",
+    "cbct_fbs_reconstruct_sharded", "cbct_cascade_run", "cbct_geometry_destroy", "cbct_geometry_query", "cbct_geometry_coarsen",
     "cbct_forward", "cbct_backproject", "cbct_backproject_eq2", "cbct_set_backprojector", "cbct_tv_prox", "cbct_prolong", "cbct_restrict", "cbct_bin2x2",
     "cbct_energy", "cbct_data_gradient", "cbct_prox_step", "cbct_fbs_reconstruct", "cbct_fbs_reconstruct_until", "cbct_forward_host", "cbct_backproject_host", "cbct_tv_prox_host",
     "cbct_fbs_reconstruct_host", "cbct_profile_enable", "cbct_profile_read", "cbct_launch_count", "cbct_device_bytes", "cbct_last_error",
 )
+
+
+# int allreduce(float *d_buf, unsigned long long count, void *user, void *cuda_stream)
+ALLREDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_ulonglong, C.c_void_p, C.c_void_p)
+
+
+class CascadeOps(C.Structure):
+    """struct cbct_cascade_ops of include/cbct.h."""
+    _L = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_int)
+    _fields_ = [("user", C.c_void_p),
+                ("level_sizes", C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_int, C.POINTER(C.c_ulonglong), C.POINTER(C.c_ulonglong))),
+                ("bin", _L), ("start", C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_int, C.c_int)), ("data_gradient", _L),
+                ("all_reduce", _L), ("prox_step", C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_int, C.c_double, C.c_double)),
+                ("prolong", _L)]
 
 
 class CbctError(RuntimeError):
@@ -49,6 +64,12 @@ def load():
     L = C.CDLL(path)
     vp, fp, dp, ip, d, f, i = C.c_void_p, C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int), C.c_double, C.c_float, C.c_int
     L.cbct_geometry_create.argtypes = [d, d, dp, i, i, i, d, d, i, i, i, d, d, d, C.POINTER(vp)]
+    L.cbct_geometry_create_ex.argtypes = [d, d, dp, i, i, i, d, d, d, d, i, i, i, d, d, d, C.POINTER(vp)]
+    L.cbct_set_detector_binning.argtypes = [vp, i]
+    L.cbct_fbs_vcycle.argtypes = [vp, fp, fp, i, i, i, i, i, i, f, f, f, f, fp, dp, vp]
+    L.cbct_fdk_reconstruct.argtypes = [vp, fp, fp, vp]
+    L.cbct_fbs_reconstruct_sharded.argtypes = [vp, fp, fp, i, ip, i, f, f, f, f, i, ALLREDUCE_FN, vp, fp, fp, vp]
+    L.cbct_cascade_run.argtypes = [C.POINTER(CascadeOps), i, ip, d, d, i, i]
     L.cbct_geometry_destroy.argtypes = [vp]
     L.cbct_geometry_destroy.restype = None
     L.cbct_geometry_query.argtypes = [vp, ip, dp]
@@ -141,7 +162,7 @@ def _host(a, n: int, name: str) -> int:
 class Geometry:
     """Owning wrapper of a cbct_geometry handle (cbct_geometry_create / _destroy)."""
 
-    def __init__(self, sad, sdd, angles, nu, nv, du, dv, nx, ny, nz, hx, hy, hz, _handle=None, _parent=None):
+    def __init__(self, sad, sdd, angles, nu, nv, du, dv, nx, ny, nz, hx, hy, hz, off_u=0.0, off_v=0.0, _handle=None, _parent=None):
         L = load()
         self._parent = _parent            # coarse handles are owned by their fine handle
         if _handle is not None:
@@ -149,9 +170,15 @@ class Geometry:
         else:
             ang = np.ascontiguousarray(angles, dtype=np.float64)
             h = C.c_void_p()
-            _check(L.cbct_geometry_create(float(sad), float(sdd), ang.ctypes.data_as(C.POINTER(C.c_double)),
-                                          int(ang.shape[0]), int(nu), int(nv), float(du), float(dv),
-                                          int(nx), int(ny), int(nz), float(hx), float(hy), float(hz), C.byref(h)))
+            if off_u == 0.0 and off_v == 0.0:
+                _check(L.cbct_geometry_create(float(sad), float(sdd), ang.ctypes.data_as(C.POINTER(C.c_double)),
+                                              int(ang.shape[0]), int(nu), int(nv), float(du), float(dv),
+                                              int(nx), int(ny), int(nz), float(hx), float(hy), float(hz), C.byref(h)))
+            else:
+                _check(L.cbct_geometry_create_ex(float(sad), float(sdd), ang.ctypes.data_as(C.POINTER(C.c_double)),
+                                                 int(ang.shape[0]), int(nu), int(nv), float(du), float(dv), float(off_u),
+                                                 float(off_v), int(nx), int(ny), int(nz), float(hx), float(hy), float(hz),
+                                                 C.byref(h)))
             self._h = h
         d6 = (C.c_int * 6)()
         s5 = (C.c_double * 5)()
@@ -162,7 +189,8 @@ class Geometry:
     @classmethod
     def from_synth(cls, g) -> "Geometry":
         """From any record with the field names of cbct_synth.Geometry."""
-        return cls(g.sad, g.sdd, g.angles, g.nu, g.nv, g.du, g.dv, g.nx, g.ny, g.nz, g.hx, g.hy, g.hz)
+        return cls(g.sad, g.sdd, g.angles, g.nu, g.nv, g.du, g.dv, g.nx, g.ny, g.nz, g.hx, g.hy, g.hz,
+                   off_u=getattr(g, "off_u", 0.0), off_v=getattr(g, "off_v", 0.0))
 
     @property
     def n_vox(self):
@@ -186,6 +214,10 @@ class Geometry:
         fl = (C.c_int * 4)()
         _check(load().cbct_geometry_coarsen(self._h, C.byref(h), fl))
         return Geometry(0, 0, None, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, _handle=h, _parent=self), tuple(bool(x) for x in fl)
+
+    def set_detector_binning(self, on: bool):
+        """Coarse levels bin the detector 2x2 (default) or keep it at full resolution; drops existing coarse levels."""
+        _check(load().cbct_set_detector_binning(self._h, 1 if on else 0))
 
     def device_bytes(self) -> int:
         return int(load().cbct_device_bytes(self._h))
@@ -265,6 +297,51 @@ def fbs_reconstruct(g: Geometry, d_Y, d_f0, n_levels, n_outer, n_inner, step, mu
                                        int(n_levels), arr, int(n_inner), float(step), float(mu), float(eps),
                                        float(omega), _dev(d_f_out, g.n_vox, "d_f_out"), tr, _stream(stream)))
     return list(tr)[:total] if trace else None
+
+
+def fbs_vcycle(g: Geometry, d_Y, d_f0, n_levels, n_cycles, nu_pre, nu_post, nu_coarse, n_inner, step, mu, eps, omega, d_f_out,
+               trace: bool = False, stream=None):
+    """FAS V-cycles around Algorithm A1 (cbct_fbs_vcycle); returns E_eps after every cycle if trace."""
+    tr = (C.c_double * max(int(n_cycles), 1))() if trace else None
+    _check(load().cbct_fbs_vcycle(g._h, _dev(d_Y, g.n_proj, "d_Y"), None if d_f0 is None else _dev(d_f0, g.n_vox, "d_f0"),
+                                  int(n_levels), int(n_cycles), int(nu_pre), int(nu_post), int(nu_coarse), int(n_inner),
+                                  float(step), float(mu), float(eps), float(omega), _dev(d_f_out, g.n_vox, "d_f_out"), tr,
+                                  _stream(stream)))
+    return list(tr)[:int(n_cycles)] if trace else None
+
+
+def fdk_reconstruct(g: Geometry, d_Y, d_vol, stream=None):
+    """The FDK baseline (cbct_fdk_reconstruct): cosine pre-weight, ramp filter along u, weighted voxel-driven backprojection."""
+    _check(load().cbct_fdk_reconstruct(g._h, _dev(d_Y, g.n_proj, "d_Y"), _dev(d_vol, g.n_vox, "d_vol"), _stream(stream)))
+
+
+def fbs_reconstruct_sharded(g: Geometry, d_Y_local, d_f0, n_levels, n_outer, n_inner, step, mu, eps, omega, n_angles_total,
+                            allreduce, d_G_scratch, d_f_out, stream=None):
+    """cbct_fbs_reconstruct_sharded.  `allreduce(count)` must sum the first `count` floats of d_G_scratch over the ranks in
+    place (None = single rank).  Argument marshalling only: the cascade and its constants live behind the C ABI."""
+    arr, _ = _outer(n_levels, n_outer)
+    gptr = _dev(d_G_scratch, g.n_vox, "d_G_scratch")
+    err = []
+
+    def _cb(d_buf, count, user, st):
+        try:
+            if int(d_buf) != gptr:
+                raise RuntimeError("all-reduce called on a buffer that is not d_G_scratch")
+            allreduce(int(count))
+            return 0
+        except Exception as e:            # never let an exception cross the C frame
+            err.append(e)
+            return 1
+
+    cb = ALLREDUCE_FN(_cb) if allreduce is not None else C.cast(None, ALLREDUCE_FN)
+    status = load().cbct_fbs_reconstruct_sharded(g._h, _dev(d_Y_local, g.n_proj, "d_Y_local"),
+                                                 None if d_f0 is None else _dev(d_f0, g.n_vox, "d_f0"), int(n_levels), arr,
+                                                 int(n_inner), float(step), float(mu), float(eps), float(omega),
+                                                 int(n_angles_total), cb, None, gptr, _dev(d_f_out, g.n_vox, "d_f_out"),
+                                                 _stream(stream))
+    if err:
+        raise err[0]
+    _check(status)
 
 
 def data_gradient(g: Geometry, d_f, d_Y, d_G, stream=None):

@@ -107,7 +107,7 @@ extern "C" cbct_status cbct_bin2x2(const cbct_geometry *fine, const float *y, fl
 }
 
 // E_eps(f); synchronises.
-static cbct_status energy_impl(cbct_geometry *g, const float *d_f, const float *d_Y, float mu, float eps,
+cbct_status op_energy(cbct_geometry *g, const float *d_f, const float *d_Y, float mu, float eps,
                                double *out3, cudaStream_t st)
 {
     CBCT_TRY(ensure_zeroed(g, &g->proj_tmp, g->n_proj(), st));
@@ -132,15 +132,18 @@ extern "C" cbct_status cbct_energy(const cbct_geometry *gc, const float *d_f, co
 {
     REQUIRE(gc && d_f && d_Y && h_out3, "cbct_energy: NULL argument");
     REQUIRE(eps >= 0.f, "cbct_energy: eps < 0");
-    return energy_impl(mut(gc), d_f, d_Y, mu, eps, h_out3, (cudaStream_t)stream);
+    return op_energy(mut(gc), d_f, d_Y, mu, eps, h_out3, (cudaStream_t)stream);
 }
 
 // ---- the two halves of an outer iteration, for drivers that put an exchange step between them (NEXT-4) ----
 extern "C" cbct_status cbct_data_gradient(const cbct_geometry *gc, const float *d_f, const float *d_Y, float *d_G, void *stream)
 {
     REQUIRE(gc && d_f && d_Y && d_G, "cbct_data_gradient: NULL argument");
-    cbct_geometry *g = mut(gc);
-    cudaStream_t st = (cudaStream_t)stream;
+    return op_data_gradient(mut(gc), d_f, d_Y, d_G, (cudaStream_t)stream);
+}
+
+cbct_status op_data_gradient(cbct_geometry *g, const float *d_f, const float *d_Y, float *d_G, cudaStream_t st)
+{
     CBCT_TRY(ensure_zeroed(g, &g->proj_tmp, g->n_proj(), st));
     CBCT_TRY(op_pad_copies(g, d_f, st));
     if (g->bp_mode == CBCT_BACKPROJECTOR_EQ2) {
@@ -176,8 +179,10 @@ extern "C" cbct_status cbct_prox_step(const cbct_geometry *gc, const float *d_f,
 // One level of Algorithm A1: f (in/out, level-sized device buffer).
 // rel_tol > 0: stop after the first iteration with ||f_new - f_old||_2 <= rel_tol ||f_new||_2 (NEXT-2; sums in fp64,
 // one stream synchronise per iteration); *iters receives the number of iterations run.
-static cbct_status fbs_level(cbct_geometry *g, const float *d_Y, float *f, int n_outer, int n_inner, float step,
-                             float mu, float eps, float omega, double *trace, float rel_tol, int *iters, cudaStream_t st)
+// tau != nullptr (FAS coarse problems, vcycle.cu): the linear term -<tau, f> joins the gradient of step 1, gv = f - c G + tau / beta.
+cbct_status op_fbs_level(cbct_geometry *g, const float *d_Y, float *f, int n_outer, int n_inner, float step,
+                         float mu, float eps, float omega, double *trace, float rel_tol, int *iters, const float *tau,
+                         cudaStream_t st)
 {
     if (rel_tol > 0.f) {
         CBCT_TRY(ensure(g, &g->vol_c, g->n_vox()));
@@ -196,28 +201,22 @@ static cbct_status fbs_level(cbct_geometry *g, const float *d_Y, float *f, int n
             // the paper's step 1 (P:87 with eq. 2): dE2/df = (2/(N_theta A)) B r, so gv = f - c (dV/(du dv)) B r
             const float c2 = (float)((double)c * (g->hx * g->hy * g->hz) / (g->du * g->dv));
             CBCT_TRY(op_forward_padded(g, g->proj_tmp, d_Y, 2, st));      // P f - Y              a1+a2
-            if (n_inner == 0) {
-                CBCT_TRY(op_backproject_eq2(g, g->proj_tmp, f, c2, 1, g->vol_a, st));
-                CBCT_CUDA(cudaMemcpyAsync(f, g->vol_a, g->n_vox() * sizeof(float), cudaMemcpyDeviceToDevice, st));
-            } else {
-                CBCT_TRY(op_backproject_eq2(g, g->proj_tmp, f, c2, 0, g->vol_a, st));          // a3 (eq. 2) + a4
-                CBCT_TRY(tv_inner(g, g->vol_a, g->vol_a, f, beta, eps, omega, n_inner, 1, st));
-            }
+            CBCT_TRY(op_backproject_eq2(g, g->proj_tmp, f, c2, n_inner == 0 && !tau, g->vol_a, st));   // a3 (eq. 2) + a4 (+ a6)
+            if (tau) CBCT_TRY(op_axpy_clamp(g, g->vol_a, tau, -1.f / beta, n_inner == 0, g->vol_a, st));
+            if (n_inner == 0) CBCT_CUDA(cudaMemcpyAsync(f, g->vol_a, g->n_vox() * sizeof(float), cudaMemcpyDeviceToDevice, st));
+            else CBCT_TRY(tv_inner(g, g->vol_a, g->vol_a, f, beta, eps, omega, n_inner, 1, st));
         } else {
             CBCT_TRY(op_forward_padded(g, g->proj_tmp, d_Y, 1, st));          // l (P f - Y)          a1+a2
             CBCT_TRY(op_backproject_prefix(g, g->proj_tmp, 0, nullptr, st));
             CBCT_TRY(op_backproject_gather(g, g->proj_tmp, st));              // P^T (P f - Y)        a3
-            if (n_inner == 0) {
-                CBCT_TRY(op_combine(g, f, c, 1, g->vol_a, st));               // max(f - c G, 0)      a4+a6
-                CBCT_CUDA(cudaMemcpyAsync(f, g->vol_a, g->n_vox() * sizeof(float), cudaMemcpyDeviceToDevice, st));
-            } else {
-                CBCT_TRY(op_combine(g, f, c, 0, g->vol_a, st));               // gv = f - c G         a4
-                CBCT_TRY(tv_inner(g, g->vol_a, g->vol_a, f, beta, eps, omega, n_inner, 1, st));   // u0 = gv (Q7); a5 + a6
-            }
+            CBCT_TRY(op_combine(g, f, c, n_inner == 0 && !tau, g->vol_a, st));    // gv = f - c G (a4), clamped (a6) if nothing follows
+            if (tau) CBCT_TRY(op_axpy_clamp(g, g->vol_a, tau, -1.f / beta, n_inner == 0, g->vol_a, st));   // + tau / beta
+            if (n_inner == 0) CBCT_CUDA(cudaMemcpyAsync(f, g->vol_a, g->n_vox() * sizeof(float), cudaMemcpyDeviceToDevice, st));
+            else CBCT_TRY(tv_inner(g, g->vol_a, g->vol_a, f, beta, eps, omega, n_inner, 1, st));   // u0 = gv (Q7); a5 + a6
         }
         if (trace) {
             double e3[3];
-            CBCT_TRY(energy_impl(g, f, d_Y, mu, eps, e3, st));
+            CBCT_TRY(op_energy(g, f, d_Y, mu, eps, e3, st));
             trace[it] = e3[0];
         }
         if (iters) *iters = it + 1;
@@ -276,8 +275,8 @@ static cbct_status fbs_cascade(const cbct_geometry *gc, const float *d_Y, const 
     int done = 0;
     for (int l = L; l >= 0; --l) {
         const int n = n_outer[L - l];
-        CBCT_TRY(fbs_level(lev[l], Y[l], F[l], n, n_inner, step, mu, eps, omega, trace ? trace + done : nullptr, rel_tol,
-                           iters_per_level ? iters_per_level + (L - l) : nullptr, st));
+        CBCT_TRY(op_fbs_level(lev[l], Y[l], F[l], n, n_inner, step, mu, eps, omega, trace ? trace + done : nullptr, rel_tol,
+                              iters_per_level ? iters_per_level + (L - l) : nullptr, nullptr, st));
         done += n;
         if (l > 0) CBCT_TRY(op_prolong(lev[l - 1], F[l], F[l - 1], st));
     }

@@ -99,7 +99,7 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
     const float x0 = cls == 0 ? maj0 : mn0, x1 = cls == 0 ? maj1 : mn1;
     const float y0 = cls == 0 ? mn0 : maj0, y1 = cls == 0 ? mn1 : maj1;
     const float ef = (float)(i - cg.ioff);
-    const float cu = 0.5f * (float)(d.nu - 1), cv = 0.5f * (float)(d.nv - 1);
+    const float cu = d.cu, cv = d.cv;                  // detector index of the central ray (shifted panels: not the middle)
     const float sdd_du = d.sdd / d.du;
     const float hz_dv = d.hz / d.dv, dv_hz = d.dv / d.hz;
     const float zk0 = (float)(k0 - d.koff) - d.zfrac;  // plane k0 in the units of z_entry(), minus zfrac

@@ -16,7 +16,7 @@ backproject_eq2_kernel(const DevGeom d, const float *__restrict__ proj, const fl
     const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 4 + threadIdx.y, k0 = blockIdx.z * KC;
     if (i >= d.nx || j >= d.ny) return;
     const float x = ((float)i - 0.5f * (float)(d.nx - 1)) * d.hx, y = ((float)j - 0.5f * (float)(d.ny - 1)) * d.hy;
-    const float cu = 0.5f * (float)(d.nu - 1), cv = 0.5f * (float)(d.nv - 1);
+    const float cu = d.cu, cv = d.cv;
     const float z0 = ((float)k0 - 0.5f * (float)(d.nz - 1)) * d.hz;
     const float inv_du = 1.f / d.du, inv_dv = 1.f / d.dv;
     float acc[KC];

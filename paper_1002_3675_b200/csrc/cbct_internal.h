@@ -45,6 +45,7 @@ struct DevGeom {
     int koff;                   // nz / 2
     float zfrac;                // nz/2.0 - koff  (0 or 0.5)
     float hx, hy, hz, du, dv, sad, sdd;
+    float cu, cv;               // detector index of the central ray: (nu-1)/2 - off_u/du, (nv-1)/2 - off_v/dv
     ClassGrid cls[2];
     const RayXY *rays;          // [na][nu]
     const float *zeta;          // [nv]  Dz(v)/hz
@@ -57,6 +58,7 @@ struct DevGeom {
 struct cbct_geometry {
     // user geometry (fp64)
     double sad, sdd, du, dv, hx, hy, hz;
+    double off_u = 0.0, off_v = 0.0;          // in-plane shift of the detector panel, mm (NEXT-3, Q19)
     int na, nu, nv, nx, ny, nz;
     std::vector<double> angles;
 
@@ -78,6 +80,8 @@ struct cbct_geometry {
     float *G_cls[2] = {nullptr, nullptr};     // per-class backprojection outputs (class 0 in [k][i][j] order)
     float *vol_a = nullptr, *vol_b = nullptr, *vol_c = nullptr, *vol_f = nullptr;   // g, u ping-pong, f
     float *Y_level = nullptr;                 // binned data for a coarse level
+    float *vc_tau = nullptr, *vc_f0 = nullptr, *vc_d = nullptr, *vc_e = nullptr;   // V-cycle: tau, restricted iterate, gradient, scratch
+    float *fdk_q = nullptr, *fdk_hk = nullptr;   // FDK: pre-weighted, filtered projections; ramp taps D h[k], k odd
     double *red_partial = nullptr;            // reduction partials
     double *red_out = nullptr;                // 2 doubles
     double *h_red = nullptr;                  // pinned host mirror of red_out
@@ -85,6 +89,7 @@ struct cbct_geometry {
     unsigned long long bytes = 0;
 
     int bp_mode = 0;                          // step 1 of A1: 0 exact transpose, 1 eq. 2 (cbct_set_backprojector)
+    int bin_detector = 1;                     // coarse levels bin the detector 2x2 (O6) or keep it at full resolution (Q20)
 
     // multigrid
     cbct_geometry *coarse = nullptr;
@@ -178,4 +183,10 @@ cbct_status op_prolong(cbct_geometry *fine, const float *c, float *f, cudaStream
 cbct_status op_restrict(cbct_geometry *fine, const float *f, float *c, cudaStream_t st);
 cbct_status op_bin2x2(cbct_geometry *fine, const float *y, float *yc, cudaStream_t st);
 cbct_status op_sumsq_diff(cbct_geometry *g, const float *a, const float *b, size_t n, double *d_out, cudaStream_t st);
+cbct_status op_tv_grad(cbct_geometry *g, const float *f, float eps, float *out, cudaStream_t st);   // tv.cu: out = grad TV_eps(f)
+// api.cu: one level of A1 (tau: optional FAS term), the data gradient P^T (P f - Y) (or eq. 2's), E_eps (synchronises)
+cbct_status op_fbs_level(cbct_geometry *g, const float *d_Y, float *f, int n_outer, int n_inner, float step, float mu, float eps,
+                         float omega, double *trace, float rel_tol, int *iters, const float *tau, cudaStream_t st);
+cbct_status op_data_gradient(cbct_geometry *g, const float *d_f, const float *d_Y, float *d_G, cudaStream_t st);
+cbct_status op_energy(cbct_geometry *g, const float *d_f, const float *d_Y, float mu, float eps, double *out3, cudaStream_t st);
 cbct_status op_axpy_clamp(cbct_geometry *g, const float *f, const float *G, float c, int clamp, float *out, cudaStream_t st);

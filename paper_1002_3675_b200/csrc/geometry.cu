@@ -43,7 +43,7 @@ static void free_handle(cbct_geometry *g)
     free_handle(g->coarse);
     void *ptrs[] = {g->d_rays, g->d_zeta, g->d_inv_zeta, g->d_dz, g->d_cs, g->d_tiles[0], g->d_tiles[1],
                     g->d_angle_has[0], g->d_angle_has[1], g->vol_pad[0], g->vol_pad[1], g->proj_tmp, g->proj_prefix,
-                    g->G_cls[0], g->G_cls[1], g->vol_a, g->vol_b, g->vol_c, g->vol_f, g->Y_level,
+                    g->G_cls[0], g->G_cls[1], g->vol_a, g->vol_b, g->vol_c, g->vol_f, g->Y_level, g->vc_tau, g->vc_f0, g->vc_d, g->vc_e, g->fdk_q, g->fdk_hk,
                     g->red_partial, g->red_out, g->host_stage_vol, g->host_stage_proj, g->host_stage_vol2};
     for (void *p : ptrs)
         if (p) cudaFree(p);
@@ -91,6 +91,8 @@ static cbct_status build_tables(cbct_geometry *g)
     d.zfrac = (float)(0.5 * g->nz - d.koff);
     d.hx = (float)g->hx; d.hy = (float)g->hy; d.hz = (float)g->hz;
     d.du = (float)g->du; d.dv = (float)g->dv; d.sad = (float)g->sad; d.sdd = (float)g->sdd;
+    d.cu = (float)(0.5 * (nu - 1) - g->off_u / g->du);
+    d.cv = (float)(0.5 * (nv - 1) - g->off_v / g->dv);
     for (int c = 0; c < 2; ++c) {
         ClassGrid &cg = d.cls[c];
         cg.nmaj = c == 0 ? g->nx : g->ny;
@@ -112,7 +114,7 @@ static cbct_status build_tables(cbct_geometry *g)
     std::vector<float> zeta(nv), inv_zeta(nv), dz(nv);
     double max_abs_zeta = 0.0;
     for (int v = 0; v < nv; ++v) {
-        double Dz = (v - 0.5 * (nv - 1)) * g->dv;
+        double Dz = (v - 0.5 * (nv - 1)) * g->dv + g->off_v;
         dz[v] = (float)Dz;
         // A ray with Dz == 0 (centre row of an odd nv) never leaves its z row.  It is given an
         // infinitesimal positive slope so that sign(sz) and sign(1/sz) agree in the kernels and a
@@ -129,7 +131,7 @@ static cbct_status build_tables(cbct_geometry *g)
         cs[a] = make_float2((float)co, (float)si);
         const double Sx = g->sad * co, Sy = g->sad * si;
         for (int u = 0; u < nu; ++u) {
-            const double uc = (u - 0.5 * (nu - 1)) * g->du;
+            const double uc = (u - 0.5 * (nu - 1)) * g->du + g->off_u;
             const double Dx = -(g->sdd - g->sad) * co - uc * si;
             const double Dy = -(g->sdd - g->sad) * si + uc * co;
             const double dXv = (Dx - Sx) / g->hx, dYv = (Dy - Sy) / g->hy;
@@ -207,13 +209,14 @@ static cbct_status build_tables(cbct_geometry *g)
 
 static cbct_status create_impl(double sad, double sdd, const double *angles, int na, int nu, int nv,
                                double du, double dv, int nx, int ny, int nz, double hx, double hy, double hz,
-                               cbct_geometry **out)
+                               double off_u, double off_v, cbct_geometry **out)
 {
     if (!out) { cbct_set_error("cbct_geometry_create: out is NULL"); return CBCT_ERR_INVALID_ARG; }
     *out = nullptr;
     if (!angles || na <= 0 || nu <= 0 || nv <= 0 || nx <= 0 || ny <= 0 || nz <= 0 ||
-        !(du > 0) || !(dv > 0) || !(hx > 0) || !(hy > 0) || !(hz > 0) || !(sad > 0) || !(sdd > sad)) {
-        cbct_set_error("cbct_geometry_create: NULL angles, non-positive size, or sad >= sdd");
+        !(du > 0) || !(dv > 0) || !(hx > 0) || !(hy > 0) || !(hz > 0) || !(sad > 0) || !(sdd > sad) ||
+        !std::isfinite(off_u) || !std::isfinite(off_v)) {
+        cbct_set_error("cbct_geometry_create: NULL angles, non-positive size, sad >= sdd, or a non-finite detector offset");
         return CBCT_ERR_INVALID_ARG;
     }
     for (int a = 0; a < na; ++a)
@@ -241,6 +244,7 @@ static cbct_status create_impl(double sad, double sdd, const double *angles, int
     cbct_geometry *g = new (std::nothrow) cbct_geometry();
     if (!g) { cbct_set_error("out of host memory"); return CBCT_ERR_ALLOC; }
     g->sad = sad; g->sdd = sdd; g->du = du; g->dv = dv; g->hx = hx; g->hy = hy; g->hz = hz;
+    g->off_u = off_u; g->off_v = off_v;
     g->na = na; g->nu = nu; g->nv = nv; g->nx = nx; g->ny = ny; g->nz = nz;
     g->angles.assign(angles, angles + na);
     cbct_status s = build_tables(g);
@@ -253,7 +257,28 @@ extern "C" cbct_status cbct_geometry_create(double sad, double sdd, const double
                                             double du, double dv, int nx, int ny, int nz,
                                             double hx, double hy, double hz, cbct_geometry **out)
 {
-    return create_impl(sad, sdd, angles, na, nu, nv, du, dv, nx, ny, nz, hx, hy, hz, out);
+    return create_impl(sad, sdd, angles, na, nu, nv, du, dv, nx, ny, nz, hx, hy, hz, 0.0, 0.0, out);
+}
+
+extern "C" cbct_status cbct_geometry_create_ex(double sad, double sdd, const double *angles, int na, int nu, int nv,
+                                               double du, double dv, double off_u, double off_v, int nx, int ny, int nz,
+                                               double hx, double hy, double hz, cbct_geometry **out)
+{
+    return create_impl(sad, sdd, angles, na, nu, nv, du, dv, nx, ny, nz, hx, hy, hz, off_u, off_v, out);
+}
+
+extern "C" cbct_status cbct_set_detector_binning(cbct_geometry *g, int on)
+{
+    if (!g) { cbct_set_error("cbct_set_detector_binning: NULL handle"); return CBCT_ERR_INVALID_ARG; }
+    if ((on != 0) == (g->bin_detector != 0)) return CBCT_OK;
+    // the coarse levels were built for the other choice: drop them (they are rebuilt on demand)
+    if (g->coarse) {
+        CBCT_CUDA(cudaDeviceSynchronize());
+        free_handle(g->coarse);
+        g->coarse = nullptr;
+    }
+    g->bin_detector = on != 0;
+    return CBCT_OK;
 }
 
 // O6 coarsening rule (Q11): axes with spacing <= sqrt(2) * min spacing halve; detector bins iff x and y did.
@@ -278,7 +303,7 @@ extern "C" cbct_status cbct_geometry_coarsen(const cbct_geometry *gc, cbct_geome
         }
         int nu = g->nu, nv = g->nv;
         double du = g->du, dv = g->dv;
-        if (fl[0] && fl[1]) {
+        if (fl[0] && fl[1] && g->bin_detector) {
             if (nu % 2 || nv % 2) {
                 cbct_set_error("cbct_geometry_coarsen: odd detector dimension on a level that bins the detector");
                 return CBCT_ERR_SHAPE;
@@ -286,9 +311,11 @@ extern "C" cbct_status cbct_geometry_coarsen(const cbct_geometry *gc, cbct_geome
             fl[3] = 1; nu /= 2; nv /= 2; du *= 2.0; dv *= 2.0;
         }
         cbct_geometry *c = nullptr;
+        // the mean position of a binned pixel pair is the binned pixel's centre with the SAME panel shift
         CBCT_TRY(create_impl(g->sad, g->sdd, g->angles.data(), g->na, nu, nv, du, dv, n[0], n[1], n[2],
-                             hn[0], hn[1], hn[2], &c));
+                             hn[0], hn[1], hn[2], g->off_u, g->off_v, &c));
         c->bp_mode = g->bp_mode;
+        c->bin_detector = g->bin_detector;
         g->coarse = c;
         std::memcpy(g->coarsen_flags, fl, sizeof(fl));
     }

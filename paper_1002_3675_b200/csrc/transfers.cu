@@ -112,12 +112,12 @@ cbct_status op_bin2x2(cbct_geometry *fine, const float *y, float *yc, cudaStream
     return CBCT_OK;
 }
 
-// out = f - c G, optionally clamped at 0 (the gradient step a4 on an already summed gradient volume)
-__global__ void __launch_bounds__(256) axpy_clamp_kernel(const float *__restrict__ f, const float *__restrict__ G, float c, int clamp,
-                                                         float *__restrict__ out, size_t n)
+// out = f - c G, optionally clamped at 0 (the gradient step a4 on an already summed gradient volume).  out may alias f or G
+// (element-wise, so no restrict qualifiers and plain loads).
+__global__ void __launch_bounds__(256) axpy_clamp_kernel(const float *f, const float *G, float c, int clamp, float *out, size_t n)
 {
     for (size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x; o < n; o += (size_t)gridDim.x * blockDim.x) {
-        float v = fmaf(-c, __ldg(G + o), __ldg(f + o));
+        float v = fmaf(-c, G[o], f[o]);
         if (clamp) v = fmaxf(v, 0.f);
         out[o] = v;
     }

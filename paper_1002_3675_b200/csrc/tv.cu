@@ -132,6 +132,33 @@ tv_value_kernel(const float *__restrict__ f, int nx, int ny, int nz, float ihx, 
     if (threadIdx.x == 0) partial[blockIdx.x] = sh[0];
 }
 
+// grad TV_eps(f) itself (O4; the FAS right-hand side of vcycle.cu needs it apart from a descent step): one thread per voxel
+// evaluates 1/n at its own site and at the three sites below it with IEEE square roots and divisions (the result feeds a
+// difference of two gradients, so it is kept at full fp32 accuracy; this kernel is not on the hot path).
+__global__ void __launch_bounds__(256)
+tv_grad_kernel(const float *__restrict__ f, float *__restrict__ out, int nx, int ny, int nz, float ihx, float ihy, float ihz, float eps2)
+{
+    const size_t n = (size_t)nx * ny * nz, sxy = (size_t)nx * ny;
+    for (size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x; o < n; o += (size_t)gridDim.x * blockDim.x) {
+        const int i = (int)(o % nx), j = (int)((o / nx) % ny), k = (int)(o / sxy);
+        auto site = [&](size_t s, int si, int sj, int sk, float &qx, float &qy, float &qz) {
+            const float c = __ldg(f + s);
+            const float dx = (si + 1 < nx) ? (__ldg(f + s + 1) - c) * ihx : 0.f;
+            const float dy = (sj + 1 < ny) ? (__ldg(f + s + nx) - c) * ihy : 0.f;
+            const float dz = (sk + 1 < nz) ? (__ldg(f + s + sxy) - c) * ihz : 0.f;
+            const float inv = 1.f / sqrtf(fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, eps2))));
+            qx = dx * inv * ihx; qy = dy * inv * ihy; qz = dz * inv * ihz;
+        };
+        float qx, qy, qz, t0, t1, t2;
+        site(o, i, j, k, qx, qy, qz);
+        float grad = -(qx + qy + qz);
+        if (i > 0) { site(o - 1, i - 1, j, k, t0, t1, t2); grad += t0; }
+        if (j > 0) { site(o - nx, i, j - 1, k, t0, t1, t2); grad += t1; }
+        if (k > 0) { site(o - sxy, i, j, k - 1, t0, t1, t2); grad += t2; }
+        out[o] = grad;
+    }
+}
+
 __global__ void final_sum_kernel(const double *__restrict__ partial, int n, double *__restrict__ out)
 {
     __shared__ double sh[256];
@@ -159,6 +186,17 @@ cbct_status op_tv_sweep(cbct_geometry *g, const float *u_in, const float *gv, fl
     tv_sweep_kernel<<<grid, 256, 0, st>>>(u_in, gv, u_out, g->nx, g->ny, g->nz, (float)(1.0 / g->hx),
                                           (float)(1.0 / g->hy), (float)(1.0 / g->hz), beta, eps * eps, dt,
                                           clamp, vec_ok);
+    CBCT_LAUNCH_CHECK();
+    return CBCT_OK;
+}
+
+cbct_status op_tv_grad(cbct_geometry *g, const float *f, float eps, float *out, cudaStream_t st)
+{
+    ProfileScope ps(5, st);
+    const size_t n = g->n_vox();
+    const int blocks = (int)((n + 255) / 256 < 148 * 16 ? (n + 255) / 256 : 148 * 16);
+    tv_grad_kernel<<<blocks, 256, 0, st>>>(f, out, g->nx, g->ny, g->nz, (float)(1.0 / g->hx), (float)(1.0 / g->hy),
+                                           (float)(1.0 / g->hz), eps * eps);
     CBCT_LAUNCH_CHECK();
     return CBCT_OK;
 }

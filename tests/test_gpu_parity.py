@@ -489,7 +489,7 @@ def test_sharded_halves_and_driver(cuda_lib, dev):
     summed where the all-reduce would be) match the oracle's reconstruction of the full scan."""
     import torch
     from oracle import fbs
-    from paper_1002_3675_b200.sharded import CudaOps, fbs_reconstruct_sharded, shard_angles
+    from paper_1002_3675_b200.sharded import fbs_reconstruct_sharded, shard_angles
     cb = cuda_lib
     cfg = make_config("c1")
     g = cfg.geom
@@ -511,25 +511,74 @@ def test_sharded_halves_and_driver(cuda_lib, dev):
         part += tmp
         shards.append((Gr, Yr))
     assert rel(part.cpu().numpy(), grad.cpu().numpy().astype(np.float64)) <= 1e-6
-    # (2) one rank
+    # (2) one rank through cbct_fbs_reconstruct_sharded: the library's own cascade, bit for bit
     args = (cfg.n_inner, cfg.step, cfg.mu, cfg.eps, cfg.omega)
     f_ref = torch.empty(G_all.vol_shape, device=dev)
     cb.fbs_reconstruct(G_all, d_Y, None, 2, [3, 2], *args, f_ref)
-    f_one = fbs_reconstruct_sharded(CudaOps(G_all, 2), d_Y, None, 2, [3, 2], *args, g.n_angles, None)
+    f_one = fbs_reconstruct_sharded(G_all, d_Y, None, 2, [3, 2], *args, g.n_angles, None)
     torch.cuda.synchronize()
     assert torch.equal(f_one, f_ref)
+    # ... and with an exchange callback that counts its calls (a one-rank "sum" leaves the buffer as it is)
+    Gs = torch.empty(G_all.vol_shape, device=dev)
+    f_cb = torch.empty(G_all.vol_shape, device=dev)
+    counts = []
+    cb.fbs_reconstruct_sharded(G_all, d_Y, None, 2, [3, 2], *args, g.n_angles, counts.append, Gs, f_cb)
+    torch.cuda.synchronize()
+    gcoarse = G_all.coarsen()[0]
+    assert counts == [gcoarse.n_vox] * 3 + [G_all.n_vox] * 2 and torch.equal(f_cb, f_ref)
+    with pytest.raises(RuntimeError):                                              # an exception in the callback surfaces in Python
+        cb.fbs_reconstruct_sharded(G_all, d_Y, None, 1, [1], *args, g.n_angles, lambda n: 1 / 0, Gs, f_cb)
 
-    # (3) two shards in one process
-    class TwoShards(CudaOps):
-        def __init__(self):
-            self.a, self.b = CudaOps(shards[0][0], 2), CudaOps(shards[1][0], 2)
-            self.cb, self.torch, self.stream, self.levels = self.a.cb, self.a.torch, None, self.a.levels
-        def bin(self, l, Ypair): return (self.a.bin(l, Ypair[0]), self.b.bin(l, Ypair[1]))
-        def data_gradient(self, l, f, Ypair): return self.a.data_gradient(l, f, Ypair[0]) + self.b.data_gradient(l, f, Ypair[1])
+    # (3) two shards in one process, driven by the library's cbct_cascade_run: each shard's halves run in the CUDA kernels,
+    # their partial gradients are added where the all-reduce would be
+    import ctypes as C
+    lv = [[G_, G_.coarsen()[0]] for G_, _ in shards]
+    Ys = [[Y_, torch.empty(l[1].proj_shape, device=dev)] for (_, Y_), l in zip(shards, lv)]
+    f = [None, None]
+    Gl = [None, None]
+    beta_seen = []
 
-    f_two = fbs_reconstruct_sharded(TwoShards(), (shards[0][1], shards[1][1]), None, 2, [3, 2], *args, g.n_angles, None)
+    def level_sizes(u, l, pv, pp):
+        pv[0], pp[0] = lv[0][l].n_vox, lv[0][l].nu * lv[0][l].nv
+        return 0
+
+    def bin_(u, l):
+        for r in range(2):
+            cb.bin2x2(lv[r][l], Ys[r][l], Ys[r][l + 1])
+        return 0
+
+    def start(u, L, have):
+        f[L] = torch.zeros(lv[0][L].vol_shape, device=dev)
+        return 0
+
+    def grad(u, l):
+        parts = []
+        for r in range(2):
+            t = torch.empty(lv[r][l].vol_shape, device=dev)
+            cb.data_gradient(lv[r][l], f[l], Ys[r][l], t)
+            parts.append(t)
+        Gl[l] = parts[0] + parts[1]
+        return 0
+
+    def prox(u, l, c, beta):
+        beta_seen.append(beta)
+        out = torch.empty_like(f[l])
+        cb.prox_step(lv[0][l], f[l], Gl[l], c, beta, cfg.eps, cfg.omega, cfg.n_inner, out)
+        f[l] = out
+        return 0
+
+    def prolong(u, l):
+        f[l - 1] = torch.empty(lv[0][l - 1].vol_shape, device=dev)
+        cb.prolong(lv[0][l - 1], f[l], f[l - 1])
+        return 0
+
+    F = dict(cb.CascadeOps._fields_)
+    ops = cb.CascadeOps(None, F["level_sizes"](level_sizes), F["bin"](bin_), F["start"](start), F["data_gradient"](grad),
+                        C.cast(None, F["all_reduce"]), F["prox_step"](prox), F["prolong"](prolong))
+    rc = cb.load().cbct_cascade_run(C.byref(ops), 2, (C.c_int * 2)(3, 2), float(cfg.step), float(cfg.mu), g.n_angles, 0)
+    assert rc == 0 and len(beta_seen) == 5
     ref2 = fbs.fbs_reconstruct(g, Y.astype(np.float64), None, 2, [3, 2], *args)
-    assert rel(f_two.cpu().numpy(), ref2) <= TOL_RECON
+    assert rel(f[0].cpu().numpy(), ref2) <= TOL_RECON
     # argument errors of the new entry points
     with pytest.raises(cb.CbctError) as ei:
         cb.prox_step(G_all, f0, grad, 1e-3, 10.0, 1e-4, 1.0, 2, grad)              # output aliases the gradient

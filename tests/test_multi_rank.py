@@ -1,5 +1,6 @@
 """The N>1 path of bench.py is "replicas only": no data-path collective, the whole-job time
 is the slowest rank's, the value the sum of all ranks' work.  Covered here on CPU with world_size 2 (gloo)."""
+import ctypes as C
 import os
 import socket
 import sys
@@ -46,60 +47,95 @@ def test_reference_arm_only_rank0_works(monkeypatch, capsys):
     assert capsys.readouterr().out == ""
 
 
-# ---- NEXT-4: angle-sharded A1 (paper_1002_3675_b200/sharded.py) over gloo, world_size 2 ---------------------
-class _OracleOps:
-    """The driver's `ops` interface on top of the fp64 oracle (tests only): lets the host-side logic of the
-    sharded driver (partition, constants, level order, the exchange) run on CPU."""
+# ---- NEXT-4: the angle-sharded cascade of the C ABI (cbct_cascade_run, csrc/cascade.cu) over gloo, world_size 2 -------
+def _oracle_cascade_ops(g, n_levels, Y_local, f0, n_inner, eps, omega, dist_):
+    """The callback table of cbct_cascade_run filled with the fp64 oracle's operators (tests only).  The level order, c and
+    beta come from the LIBRARY; this side only keeps the per-level state and applies the operators it is asked for."""
+    import numpy as np
+    import oracle as o
+    from oracle import fbs
+    from paper_1002_3675_b200.binding import CascadeOps
+    geoms, axes, binned = fbs.level_geometries(g, n_levels)
+    st = {"Y": [np.asarray(Y_local, dtype=np.float64)] + [None] * (n_levels - 1), "f": [None] * n_levels, "G": [None] * n_levels,
+          "calls": []}
 
-    def __init__(self, g, n_levels):
-        from oracle import fbs
-        self.fbs = fbs
-        self.geoms, self.axes, self.binned = fbs.level_geometries(g, n_levels)
+    def level_sizes(user, l, p_nvox, p_npix):
+        p_nvox[0], p_npix[0] = geoms[l].n_vox, geoms[l].nu * geoms[l].nv
+        return 0
 
-    def n_vox(self, l): return self.geoms[l].n_vox
-    def n_pix(self, l): return self.geoms[l].nu * self.geoms[l].nv
-    def zeros(self, l):
-        import numpy as np
-        return np.zeros(self.geoms[l].vol_shape)
-    def bin(self, l, Y): return self.fbs.bin2x2(Y) if self.binned[l] else Y
-    def restrict(self, l, f): return self.fbs.restrict_volume(f, self.axes[l])
-    def prolong(self, l, fc): return self.fbs.prolong(fc, self.axes[l])
-    def data_gradient(self, l, f, Y):
-        import oracle as o
-        return o.backproject(self.geoms[l], o.forward(self.geoms[l], f) - Y)
-    def all_reduce(self, G, dist_):
-        if dist_ is not None:
-            t = torch.from_numpy(G)
-            dist_.all_reduce(t, op=dist_.ReduceOp.SUM)          # in place: t shares G's memory
-    def prox_step(self, l, f, G, c, beta, eps, omega, n_inner):
-        import numpy as np
-        import oracle as o
-        gv = f - c * G
-        return np.maximum(o.tv_prox(self.geoms[l], gv, gv, beta, eps, omega, n_inner), 0.0)
+    def bin_(user, l):
+        st["Y"][l + 1] = fbs.bin2x2(st["Y"][l]) if binned[l] else st["Y"][l]
+        return 0
+
+    def start(user, L, have_f0):
+        if not have_f0:
+            st["f"][L] = np.zeros(geoms[L].vol_shape)
+        else:
+            f = np.asarray(f0, dtype=np.float64)
+            for l in range(L):
+                f = fbs.restrict_volume(f, axes[l])
+            st["f"][L] = f
+        return 0
+
+    def data_gradient(user, l):
+        st["G"][l] = o.backproject(geoms[l], o.forward(geoms[l], st["f"][l]) - st["Y"][l])
+        st["calls"].append(("grad", l))
+        return 0
+
+    def all_reduce(user, l):
+        t = torch.from_numpy(st["G"][l])
+        dist_.all_reduce(t, op=dist_.ReduceOp.SUM)              # in place: t shares G's memory
+        st["calls"].append(("allreduce", l))
+        return 0
+
+    def prox_step(user, l, c, beta):
+        gv = st["f"][l] - c * st["G"][l]
+        st["f"][l] = np.maximum(o.tv_prox(geoms[l], gv, gv, beta, eps, omega, n_inner), 0.0)
+        st["calls"].append(("prox", l, c, beta))
+        return 0
+
+    def prolong(user, l):
+        st["f"][l - 1] = fbs.prolong(st["f"][l], axes[l - 1])
+        return 0
+
+    F = dict(CascadeOps._fields_)
+    ops = CascadeOps(None, F["level_sizes"](level_sizes), F["bin"](bin_), F["start"](start), F["data_gradient"](data_gradient),
+                     F["all_reduce"](all_reduce) if dist_ is not None else C.cast(None, F["all_reduce"]),
+                     F["prox_step"](prox_step), F["prolong"](prolong))
+    return ops, st
+
+
+def _run_cascade(ops, n_outer, step, mu, n_angles_total, have_f0=0):
+    import paper_1002_3675_b200 as cb
+    L = cb.load()                                               # loads on a CPU-only box; cbct_cascade_run makes no CUDA call
+    arr = (C.c_int * len(n_outer))(*n_outer)
+    return L.cbct_cascade_run(C.byref(ops), len(n_outer), arr, float(step), float(mu), int(n_angles_total), int(have_f0))
 
 
 def _sharded_worker(rank, world, port, out):
     sys.path.insert(0, ROOT)
     import numpy as np
     from cbct_synth import make_config
-    from paper_1002_3675_b200.sharded import fbs_reconstruct_sharded, shard_angles
+    from paper_1002_3675_b200.sharded import shard_angles
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world),
                       OMP_NUM_THREADS="2")
     dist.init_process_group("gloo", rank=rank, world_size=world)
-    cfg = make_config("c1", shrink=2)
+    cfg = make_config("c3", shrink=16)                          # noisy data: the shards must partition ONE noisy scan
     g, Y = cfg.geom, cfg.projections()
     mine = shard_angles(g.n_angles, rank, world)
-    ops = _OracleOps(g.with_angles(g.angles[mine]), 2)
-    f = fbs_reconstruct_sharded(ops, np.ascontiguousarray(Y[mine]), None, 2, [3, 2], cfg.n_inner, cfg.step, cfg.mu,
-                                cfg.eps, cfg.omega, g.n_angles, dist)
-    out[rank] = f
+    assert np.array_equal(cfg.projections(mine), Y[mine])
+    ops, st = _oracle_cascade_ops(g.with_angles(g.angles[mine]), 2, np.ascontiguousarray(Y[mine]), None, cfg.n_inner, cfg.eps,
+                                  cfg.omega, dist)
+    rc = _run_cascade(ops, [3, 2], cfg.step, cfg.mu, g.n_angles)
+    out[rank] = (rc, st["f"][0], st["calls"])
     dist.barrier()
     dist.destroy_process_group()
 
 
-def test_angle_sharded_driver_equals_the_single_rank_reconstruction():
-    """Two ranks, each with every second angle and its share of Y: after the per-iteration all-reduce of the
-    gradient volume both hold the reconstruction of the full scan (P^T over a subset is an exact partial sum)."""
+def test_angle_sharded_cascade_of_the_library_equals_the_single_rank_reconstruction():
+    """Two ranks, each with every second angle and its share of Y, driven by the LIBRARY's cbct_cascade_run: after the
+    per-iteration all-reduce of the gradient volume both hold the reconstruction of the full scan (P^T over a subset is an
+    exact partial sum).  Also checks the constants the library hands to the prox step and the order of its calls."""
     import numpy as np
     sys.path.insert(0, ROOT)
     from cbct_synth import make_config
@@ -110,13 +146,43 @@ def test_angle_sharded_driver_equals_the_single_rank_reconstruction():
         port = s.getsockname()[1]
     out = mp.Manager().dict()
     mp.spawn(_sharded_worker, args=(2, port, out), nprocs=2, join=True)
-    cfg = make_config("c1", shrink=2)
-    ref = fbs.fbs_reconstruct(cfg.geom, cfg.projections(), None, 2, [3, 2], cfg.n_inner, cfg.step, cfg.mu, cfg.eps, cfg.omega)
-    assert np.array_equal(out[0], out[1])                       # every rank applies the same prox step to the same sum
-    assert np.linalg.norm(out[0] - ref) <= 1e-12 * np.linalg.norm(ref)
+    cfg = make_config("c3", shrink=16)
+    g = cfg.geom
+    ref = fbs.fbs_reconstruct(g, cfg.projections(), None, 2, [3, 2], cfg.n_inner, cfg.step, cfg.mu, cfg.eps, cfg.omega)
+    assert out[0][0] == 0 and out[1][0] == 0
+    assert np.array_equal(out[0][1], out[1][1])                 # every rank applies the same prox step to the same sum
+    assert np.linalg.norm(out[0][1] - ref) <= 1e-12 * np.linalg.norm(ref)
+    calls = out[0][2]
+    assert [c[0] for c in calls] == ["grad", "allreduce", "prox"] * 5 and [c[1] for c in calls] == [1] * 9 + [0] * 6
+    gc = fbs.coarsen_geometry(g)[0]
+    for (_, l, c, beta), gl in zip([c for c in calls if c[0] == "prox"], [gc] * 3 + [g] * 2):
+        assert c == 2.0 * cfg.step * gl.n_vox / (g.n_angles * gl.n_pix) and beta == cfg.mu / cfg.step
     # the partition covers every angle exactly once
     idx = np.sort(np.concatenate([shard_angles(17, r, 3) for r in range(3)]))
     assert np.array_equal(idx, np.arange(17))
+
+
+def test_cascade_run_single_rank_and_errors():
+    """One rank, no exchange callback: cbct_cascade_run with the oracle's operators IS the oracle's cascade (with a caller's
+    f0 restricted down); bad arguments and failing callbacks come back as status codes."""
+    import numpy as np
+    sys.path.insert(0, ROOT)
+    import paper_1002_3675_b200 as cb
+    from cbct_synth import make_config
+    from oracle import fbs
+    cfg = make_config("c1", shrink=2)
+    g, Y = cfg.geom, cfg.projections()
+    f0 = np.abs(np.random.default_rng(0).normal(size=g.vol_shape)) * 0.01
+    ops, st = _oracle_cascade_ops(g, 2, Y, f0, cfg.n_inner, cfg.eps, cfg.omega, None)
+    assert _run_cascade(ops, [2, 3], cfg.step, cfg.mu, g.n_angles, have_f0=1) == 0
+    ref = fbs.fbs_reconstruct(g, Y, f0, 2, [2, 3], cfg.n_inner, cfg.step, cfg.mu, cfg.eps, cfg.omega)
+    assert np.array_equal(st["f"][0], ref)
+    assert all(c[0] != "allreduce" for c in st["calls"])
+    assert _run_cascade(ops, [2, -1], cfg.step, cfg.mu, g.n_angles) == 1          # negative count
+    assert _run_cascade(ops, [1, 1], 0.0, cfg.mu, g.n_angles) == 1                 # step <= 0
+    F = dict(cb.CascadeOps._fields_)
+    ops.prox_step = F["prox_step"](lambda u, l, c, b: 3)                           # a callback's status is passed through
+    assert _run_cascade(ops, [1, 1], cfg.step, cfg.mu, g.n_angles) == 3
 
 
 def test_bench_gpus_n_starts_n_ranks_by_itself():
