@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(128) prefix_kernel(const DevGeom d, const floa
 
 
 #ifndef CBCT_BP_VOTE
-#define CBCT_BP_VOTE 1
+#define CBCT_BP_VOTE 0
 #endif
 
 template <int KC, int BI>
