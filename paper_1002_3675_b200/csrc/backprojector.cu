@@ -77,8 +77,11 @@ __global__ void __launch_bounds__(128) prefix_kernel(const DevGeom d, const floa
 #define CBCT_BP_VOTE 0
 #endif
 
+#ifndef CBCT_BP_MINB
+#define CBCT_BP_MINB 8
+#endif
 template <int KC, int BI>
-__global__ void __launch_bounds__(32 * BI)
+__global__ void __launch_bounds__(32 * BI, CBCT_BP_MINB)
 backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restrict__ angle_has,
                    const float *__restrict__ rs, const float2 *__restrict__ C, float *__restrict__ G)
 {
@@ -135,7 +138,10 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
             const float T = fmaf(ef, r.dt, r.tc), Tn = fmaf(ef + 1.f, r.dt, r.tc);   // entry / exit ray parameter
             const float cT = hz_dv * rcp_approx(T), cTn = hz_dv * rcp_approx(Tn);     // d v / d z at entry / exit (T > 0)
             // 32-bit element offsets of (a, v = 0, u) in the prefix sums and in the projections (checked at geometry creation)
-            const int offC = a * (d.nv + 1) * d.nu + u, offR = a * d.nv * d.nu + u;
+            // byte offsets: one IMAD.WIDE (row * pitch + base) forms the address of a row's element
+            const char *Cu = reinterpret_cast<const char *>(C + (a * (d.nv + 1) * d.nu + u));
+            const char *Ru = reinterpret_cast<const char *>(rs + (a * d.nv * d.nu + u));
+            const int pitchC = d.nu * (int)sizeof(float2), pitchR = d.nu * (int)sizeof(float);
             const float Tdv = T * dv_hz, dtdv = r.dt * dv_hz;                         // T zeta(v) = Tdv (v - cv), dt zeta(v) = dtdv (v - cv)
             // entry and exit bounds of a plane less than one detector row apart on every plane of the chunk: at most one
             // ray crosses a plane inside the slab, and the loop over further crossing rays is compiled out
@@ -157,7 +163,7 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
                         vT = min(max(vT, 0), d.nv);
                         vTn = min(max(vTn, 0), d.nv);
                     }
-                    const float2 c2 = __ldg(C + (offC + vT * d.nu));
+                    const float2 c2 = __ldg(reinterpret_cast<const float2 *>(Cu + (long long)vT * pitchC));
                     // rays crossing plane k0+q inside the slab: v in [min(vT,vTn), max(vT,vTn)) (y = 0 stands in if there is none).
                     // b = lambda at which the ray meets the plane: T(lambda) zeta(v) = zk with T(lambda) = T + lambda dt and
                     // zeta(v) = (v - cv) dv / hz, i.e. b = (zk - T zeta(v)) / (dt zeta(v)), the projector's b with its numerator
@@ -172,14 +178,14 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
                         const float bq = __saturatef(fmaf(-Tdv, vf, zk) * rcp_approx(vf * dtdv));
                         // rising iff dt zeta(v) > 0: move the sign bit of dt zeta(v) onto y
                         float yq = 0.f;
-                        if (dlt != 0) yq = __ldg(rs + (offR + vs * d.nu));
+                        if (dlt != 0) yq = __ldg(reinterpret_cast<const float *>(Ru + (long long)vs * pitchR));
                         yq = __int_as_float(__float_as_int(yq) ^ (__float_as_int(vf * dtdv) & 0x80000000));
                         up = fmaxf(0.f, l1 - fmaxf(l0, bq)) * yq;
                         if constexpr (MULTI) {
                             for (int v = vs + 1; v < vs + abs(dlt); ++v) {   // further rays crossing this plane (fine detector rows)
                                 const float vf2 = (float)v - cv;
                                 const float b2 = __saturatef(fmaf(-Tdv, vf2, zk) * rcp_approx(vf2 * dtdv));
-                                const float y2 = __ldg(rs + (offR + v * d.nu));
+                                const float y2 = __ldg(reinterpret_cast<const float *>(Ru + (long long)v * pitchR));
                                 up = fmaf(fmaxf(0.f, l1 - fmaxf(l0, b2)), __int_as_float(__float_as_int(y2) ^ (__float_as_int(vf * dtdv) & 0x80000000)), up);
                             }
                         }

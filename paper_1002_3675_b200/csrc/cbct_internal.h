@@ -177,6 +177,8 @@ cbct_status op_tv_sweep(cbct_geometry *g, const float *u_in, const float *gv, fl
                         float beta, float eps, float dt, int clamp, cudaStream_t st);
 cbct_status op_tv_sweep_rows(cbct_geometry *g, const float *u_in, const float *gv, float *u_out, float beta, float eps,
                              float dt, int clamp, cudaStream_t st, int *done);   // tv_rows.cu
+cbct_status op_tv_sweep_tma(cbct_geometry *g, const float *u_in, const float *gv, float *u_out, float beta, float eps,
+                            float dt, int clamp, cudaStream_t st, int *done);    // tv_tma.cu
 cbct_status op_tv_value(cbct_geometry *g, const float *f, float eps, double *d_out, cudaStream_t st);
 // transfers.cu
 cbct_status op_prolong(cbct_geometry *fine, const float *c, float *f, cudaStream_t st);

@@ -179,6 +179,10 @@ cbct_status op_tv_sweep(cbct_geometry *g, const float *u_in, const float *gv, fl
 {
     ProfileScope ps(5, st);
     int done = 0;
+#ifndef CBCT_TV_NO_TMA
+    CBCT_TRY(op_tv_sweep_tma(g, u_in, gv, u_out, beta, eps, dt, clamp, st, &done));    // nx <= 512, nx % 4 == 0: TMA-fed rows (tv_tma.cu)
+    if (done) return CBCT_OK;
+#endif
     CBCT_TRY(op_tv_sweep_rows(g, u_in, gv, u_out, beta, eps, dt, clamp, st, &done));   // nx <= 512: row-streaming kernel (tv_rows.cu)
     if (done) return CBCT_OK;
     dim3 grid((g->nx + TX - 1) / TX, (g->ny + TY - 1) / TY, (g->nz + TZ - 1) / TZ);

@@ -136,6 +136,7 @@ def test_backproject_of_unit_projections_matches_brute_force_clip(cuda_lib, dev)
                                      # per lane, vector rows of 4, 8, 16; and the tile kernel for nx > 512 (ragged and full tiles)
                                      ((102, 9, 7), (1.0, 1.0, 2.0)), ((130, 7, 6), (0.5, 0.5, 2.5)), ((258, 6, 5), (1.0, 1.0, 1.0)),
                                      ((100, 13, 9), (1.0, 1.0, 1.0)), ((200, 11, 5), (1.0, 1.0, 1.0)), ((512, 12, 6), (0.5, 0.5, 2.5)),
+                                     ((320, 9, 7), (1.0, 1.0, 1.0)), ((36, 5, 3), (1.0, 1.0, 1.0)), ((256, 40, 21), (1.0, 1.0, 1.0)), ((448, 23, 9), (0.5, 0.5, 2.5)),
                                      ((516, 10, 9), (1.0, 1.0, 1.0)), ((1024, 9, 10), (0.5, 0.5, 0.5))])
 def test_tv_prox(cuda_lib, dev, shape, h):
     import torch
