@@ -109,6 +109,14 @@ cbct_status cbct_set_detector_binning(cbct_geometry *g, int on);
 cbct_status cbct_forward(const cbct_geometry *g, const float *d_vol, float *d_proj, void *cuda_stream);
 
 /*
+ * Which projector kernel cbct_forward and the cascades use on this handle (and its coarse levels): 0 (default) the march that
+ * reads the padded volume copies through the L1 cache, 1 the same march fed by TMA-staged shared-memory bricks (falls back
+ * to 0 where a brick would not fit).  Same rays, same arithmetic, same results to rounding order; see DESIGN.md for the
+ * measured comparison.
+ */
+cbct_status cbct_set_projector_staging(cbct_geometry *g, int on);
+
+/*
  * a3. Backprojection G = P^T y — the exact transpose of cbct_forward's matrix ("P^T denotes a
  * matrix transpose"; O2), evaluated as a race-free gather (the paper's "memory conflict" remark,
  * P:95): <P x, y> = <x, P^T y> up to fp32 rounding.  d_vol is overwritten.

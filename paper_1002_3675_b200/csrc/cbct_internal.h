@@ -3,7 +3,9 @@
 #include <cuda_runtime.h>
 
 #include <cstdint>
+#include <cmath>
 #include <cstdio>
+#include <algorithm>
 #include <vector>
 
 #include "../../include/cbct.h"
@@ -89,6 +91,8 @@ struct cbct_geometry {
     unsigned long long bytes = 0;
 
     int bp_mode = 0;                          // step 1 of A1: 0 exact transpose, 1 eq. 2 (cbct_set_backprojector)
+    int fw_staged = 0;                        // projector: 1 = TMA-staged bricks (projector_tma.cu), 0 = __ldg march
+    int fw_bj[2] = {0, 0}, fw_bk[2] = {0, 0};  // brick spans per class (0 = not computed yet)
     int bin_detector = 1;                     // coarse levels bin the detector 2x2 (O6) or keep it at full resolution (Q20)
 
     // multigrid
@@ -161,6 +165,7 @@ inline size_t pad_elems(const cbct_geometry *g, int c)
 cbct_status op_pad_copies(cbct_geometry *g, const float *d_vol, cudaStream_t st);
 // mode 0: out = P f ; mode 1: out = l * (P f - Y)  (scaled residual for the gather) ; mode 2: out = P f - Y
 cbct_status op_forward_padded(cbct_geometry *g, float *d_out, const float *d_Y, int mode, cudaStream_t st);
+cbct_status op_forward_padded_tma(cbct_geometry *g, float *d_out, const float *d_Y, int mode, cudaStream_t st, int *done);   // projector_tma.cu
 // backprojector.cu : gathers of the (already l-scaled) projections into G_cls[0], G_cls[1].
 // op_backproject_prefix builds the prefix sums along v that the gather reads (scale != 0: of l * d_in,
 // also written to d_rs_out); it must run on the same projections before op_backproject_gather.

@@ -316,6 +316,7 @@ extern "C" cbct_status cbct_geometry_coarsen(const cbct_geometry *gc, cbct_geome
                              hn[0], hn[1], hn[2], g->off_u, g->off_v, &c));
         c->bp_mode = g->bp_mode;
         c->bin_detector = g->bin_detector;
+        c->fw_staged = g->fw_staged;
         g->coarse = c;
         std::memcpy(g->coarsen_flags, fl, sizeof(fl));
     }

@@ -182,6 +182,11 @@ cbct_status op_forward_padded(cbct_geometry *g, float *d_out, const float *d_Y, 
 #define CBCT_FW_WARPS 4
 #endif
     constexpr int V = CBCT_FW_V, WARPS = CBCT_FW_WARPS;
+    if (g->fw_staged) {
+        int done = 0;
+        CBCT_TRY(op_forward_padded_tma(g, d_out, d_Y, mode, st, &done));
+        if (done) return CBCT_OK;
+    }
     ProfileScope ps(1, st);
     // every ray belongs to a tile of its class (geometry.cu), so every output element is written: 0 / -Y / -l Y for a
     // ray that misses the volume
