@@ -83,12 +83,16 @@ __global__ void __launch_bounds__(128) prefix_kernel(const DevGeom d, const floa
 template <int KC, int BI>
 __global__ void __launch_bounds__(32 * BI, CBCT_BP_MINB)
 backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restrict__ angle_has,
-                   const float *__restrict__ rs, const float2 *__restrict__ C, float *__restrict__ G)
+                   const float *__restrict__ rs, const float2 *__restrict__ C, float *__restrict__ G, const int parts)
 {
     const ClassGrid cg = d.cls[cls];
     const int j = blockIdx.x * 32 + threadIdx.x;      // minor index
     const int i = blockIdx.y * BI + threadIdx.y;      // major index = slab
-    const int k0 = blockIdx.z * KC;
+    // small volumes: the angle list is dealt out over `parts` CTAs per column chunk (part p takes angles p, p + parts, ...),
+    // each writing its own partial volume; op_combine adds the partial volumes in the order of p
+    const int kchunks = gridDim.z / parts, part = blockIdx.z / kchunks;
+    const int k0 = (blockIdx.z - part * kchunks) * KC;
+    G += (size_t)part * d.nx * d.ny * d.nz;
     if (i >= cg.nmaj) return;                          // warp-uniform
     const bool valid = j < cg.nmin;
 
@@ -107,7 +111,7 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
     const float hz_dv = d.hz / d.dv, dv_hz = d.dv / d.hz;
     const float zk0 = (float)(k0 - d.koff) - d.zfrac;  // plane k0 in the units of z_entry(), minus zfrac
 
-    for (int a = 0; a < d.na; ++a) {
+    for (int a = part; a < d.na; a += parts) {
         if (!angle_has[a]) continue;                   // uniform
         const float2 cs = __ldg(d.cs + a);
         float umin = 3e38f, umax = -3e38f;
@@ -230,12 +234,26 @@ cbct_status op_backproject_gather(cbct_geometry *g, const float *d_scaled, cudaS
 #endif
     constexpr int KC = CBCT_BP_KC, BI = CBCT_BP_BI;
     ProfileScope ps(3, st);
+    // A small volume has too few voxel columns to fill the GPU (c1: 16 CTAs per class, 70 us per launch whatever the clock):
+    // the angles are then dealt out over up to 8 CTAs per column chunk, aiming at two CTAs per SM
+    g->bp_parts = 1;
+    {
+        int dev = 0, sms = 148;
+        if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        const ClassGrid &cg = g->dev.cls[0];
+        const long ctas = (long)((cg.nmin + 31) / 32) * ((cg.nmaj + BI - 1) / BI) * ((g->nz + KC - 1) / KC);
+        while (g->bp_parts < 8 && ctas * g->bp_parts < 2L * sms && 2 * g->bp_parts <= g->na) g->bp_parts *= 2;
+    }
     for (int c = 0; c < 2; ++c) {
         if (g->n_tiles[c] == 0) continue;
-        CBCT_TRY(ensure(g, &g->G_cls[c], g->n_vox()));
+        if (g->G_parts_alloc[c] < g->bp_parts) {
+            if (g->G_cls[c]) { CBCT_CUDA(cudaStreamSynchronize(st)); cudaFree(g->G_cls[c]); g->bytes -= g->n_vox() * sizeof(float) * g->G_parts_alloc[c]; g->G_cls[c] = nullptr; }
+            CBCT_TRY(ensure(g, &g->G_cls[c], g->n_vox() * g->bp_parts));
+            g->G_parts_alloc[c] = g->bp_parts;
+        }
         const ClassGrid &cg = g->dev.cls[c];
-        dim3 grid((cg.nmin + 31) / 32, (cg.nmaj + BI - 1) / BI, (g->nz + KC - 1) / KC), block(32, BI);
-        backproject_kernel<KC, BI><<<grid, block, 0, st>>>(g->dev, c, g->d_angle_has[c], d_scaled, g->proj_prefix, g->G_cls[c]);
+        dim3 grid((cg.nmin + 31) / 32, (cg.nmaj + BI - 1) / BI, ((g->nz + KC - 1) / KC) * g->bp_parts), block(32, BI);
+        backproject_kernel<KC, BI><<<grid, block, 0, st>>>(g->dev, c, g->d_angle_has[c], d_scaled, g->proj_prefix, g->G_cls[c], g->bp_parts);
         CBCT_LAUNCH_CHECK();
     }
     return CBCT_OK;
@@ -245,7 +263,7 @@ cbct_status op_backproject_gather(cbct_geometry *g, const float *d_scaled, cudaS
 // transpose-add that the two-class gather needs anyway.
 __global__ void __launch_bounds__(256) combine_kernel(const float *__restrict__ G0, const float *__restrict__ G1,
                                                       const float *__restrict__ f, float c, int clamp,
-                                                      float *__restrict__ out, int nx, int ny)
+                                                      float *__restrict__ out, int nx, int ny, int parts, size_t nvox)
 {
     __shared__ float tile[32][33];
     const int k = blockIdx.z;
@@ -255,7 +273,10 @@ __global__ void __launch_bounds__(256) combine_kernel(const float *__restrict__ 
         // G0 is [k][x][y]: read rows of constant x
         for (int r = threadIdx.y; r < 32; r += 8) {
             int i = i0 + r, j = j0 + threadIdx.x;
-            tile[r][threadIdx.x] = (i < nx && j < ny) ? __ldg(G0 + plane + (size_t)i * ny + j) : 0.f;
+            float v = 0.f;
+            if (i < nx && j < ny)
+                for (int p = 0; p < parts; ++p) v += __ldg(G0 + p * nvox + plane + (size_t)i * ny + j);
+            tile[r][threadIdx.x] = v;
         }
         __syncthreads();
     }
@@ -264,7 +285,8 @@ __global__ void __launch_bounds__(256) combine_kernel(const float *__restrict__ 
         if (j < ny && i < nx) {
             const size_t o = plane + (size_t)j * nx + i;
             float gsum = G0 ? tile[threadIdx.x][r] : 0.f;
-            if (G1) gsum += __ldg(G1 + o);
+            if (G1)
+                for (int p = 0; p < parts; ++p) gsum += __ldg(G1 + p * nvox + o);
             float val = gsum;
             if (f) {
                 val = fmaf(-c, gsum, __ldg(f + o));
@@ -281,7 +303,7 @@ cbct_status op_combine(cbct_geometry *g, const float *f, float c, int clamp, flo
     const float *G0 = g->n_tiles[0] > 0 ? g->G_cls[0] : nullptr;
     const float *G1 = g->n_tiles[1] > 0 ? g->G_cls[1] : nullptr;
     dim3 grid((g->nx + 31) / 32, (g->ny + 31) / 32, g->nz), block(32, 8);
-    combine_kernel<<<grid, block, 0, st>>>(G0, G1, f, c, clamp, out, g->nx, g->ny);
+    combine_kernel<<<grid, block, 0, st>>>(G0, G1, f, c, clamp, out, g->nx, g->ny, g->bp_parts, g->n_vox());
     CBCT_LAUNCH_CHECK();
     return CBCT_OK;
 }

@@ -2,6 +2,8 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <atomic>
+
 #include <cstdint>
 #include <cmath>
 #include <cstdio>
@@ -90,6 +92,7 @@ struct cbct_geometry {
     float *host_stage_vol = nullptr, *host_stage_proj = nullptr, *host_stage_vol2 = nullptr;  // device staging for *_host
     unsigned long long bytes = 0;
 
+    int bp_parts = 1, G_parts_alloc[2] = {0, 0};   // gather: angle parts per column chunk (small volumes), partial volumes allocated
     int bp_mode = 0;                          // step 1 of A1: 0 exact transpose, 1 eq. 2 (cbct_set_backprojector)
     int fw_staged = 0;                        // projector: 1 = TMA-staged bricks (projector_tma.cu), 0 = __ldg march
     int fw_bj[2] = {0, 0}, fw_bk[2] = {0, 0};  // brick spans per class (0 = not computed yet)
@@ -120,7 +123,7 @@ void cbct_set_error(const char *fmt, ...);
         if (s_ != CBCT_OK) return s_;         \
     } while (0)
 
-extern unsigned long long g_cbct_launches;
+extern std::atomic<unsigned long long> g_cbct_launches;
 #define CBCT_LAUNCH_CHECK()                                                      \
     do {                                                                         \
         ++g_cbct_launches;                                                       \

@@ -7,7 +7,7 @@
 
 #include "cbct_internal.h"
 
-unsigned long long g_cbct_launches = 0;
+std::atomic<unsigned long long> g_cbct_launches{0};
 static thread_local char t_err[512] = "";
 
 void cbct_set_error(const char *fmt, ...)
@@ -19,7 +19,7 @@ void cbct_set_error(const char *fmt, ...)
 }
 
 extern "C" const char *cbct_last_error(void) { return t_err; }
-extern "C" unsigned long long cbct_launch_count(void) { return g_cbct_launches; }
+extern "C" unsigned long long cbct_launch_count(void) { return g_cbct_launches.load(); }
 
 cbct_status cbct_dev_alloc(cbct_geometry *g, void **p, size_t bytes, bool zero, cudaStream_t st)
 {
