@@ -108,19 +108,13 @@ class ClockSampler:
         return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def level_dims(g, levels):
-    """(n_vox, n_rays) per level under the O6 coarsening rule (restated; no arithmetic of the method)."""
-    out = []
-    nx, ny, nz, nu, nv = g.nx, g.ny, g.nz, g.nu, g.nv
-    hx, hy, hz = g.hx, g.hy, g.hz
-    for _ in range(levels):
-        out.append((nx * ny * nz, g.n_angles * nu * nv))
-        m = min(hx, hy, hz)
-        ax = [h <= 2 ** 0.5 * m * (1 + 1e-9) for h in (hx, hy, hz)]
-        if ax[0]: nx //= 2; hx *= 2
-        if ax[1]: ny //= 2; hy *= 2
-        if ax[2]: nz //= 2; hz *= 2
-        if ax[0] and ax[1]: nu //= 2; nv //= 2
+def level_dims(G, levels):
+    """(n_vox, n_rays) per level, asked of the library's own coarse-level handles (cbct_geometry_coarsen)."""
+    out, cur = [], G
+    for l in range(levels):
+        out.append((cur.n_vox, cur.n_proj))
+        if l + 1 < levels:
+            cur = cur.coarsen()[0]
     return out
 
 
@@ -163,7 +157,7 @@ def run_gpu(args):
     Y = np.ascontiguousarray(cfg.projections(), dtype=np.float32)
     G = cb.Geometry.from_synth(g)
     n_outer = [1] * LEVELS
-    lv = level_dims(g, LEVELS)
+    lv = level_dims(G, LEVELS)
     updates = 2.0 * sum(nvox * g.n_angles for nvox, _ in lv)
 
     st = torch.cuda.Stream(device=dev)
@@ -271,7 +265,12 @@ def run_gpu(args):
 
     extra = {"gups_forward": gups_p, "gups_backproject": gups_bp, "tv_GBps": tv_gbs,
              "tv_frac_of_hbm": tv_gbs / pk["hbm_gbs"],
+             "tv_note": "tv_GBps is the c2 step's figure (256^3 + 128^3 volumes of 67 + 8 MB: partly L2-resident between sweeps, so "
+                        "not an HBM fraction); tv_GBps_512cube is the same kernel on 512^3 volumes (537 MB each, nothing resident)",
              "ms_per_step_by_kernel": {k: v[0] / K for k, v in prof.items()}}
+    if not args.no_recon and world == 1:
+        tvb = time_tv_512(cb, dev, st, flush)
+        extra.update(tv_GBps_512cube=tvb, tv_512cube_frac_of_hbm=tvb / pk["hbm_gbs"])
     if not args.no_recon and world == 1:
         extra["sec_per_fbs_recon_c3"] = time_c3_recon(cb, dev, st)
         # NEXT-1 (not part of `value`): the paper's eq. 2 backprojector, alone at c2 and inside the c3 reconstruction
@@ -288,6 +287,8 @@ def run_gpu(args):
             eb.record(st)
         torch.cuda.synchronize()
         extra["gups_backproject_eq2"] = g.n_vox * g.n_angles / (ea.elapsed_time(eb) / 5e3) / 1e9
+        # NEXT-4 (not part of `value`): the FDK baseline on c3's data, beside the FBS reconstruction of the same scan
+        extra["sec_fdk_c3"] = time_c3_fdk(cb, dev, st)
     cpu = cpu_baseline_sample(cfg, n_angles=args.cpu_angles) if world == 1 and not args.no_cpu else None
 
     line = {
@@ -357,7 +358,7 @@ def run_sharded(args):
         torch.cuda.synchronize()
     t = max_over_ranks(sum(a.elapsed_time(b) for a, b in ev) / 1e3, dist, dev)
     if rank == 0:
-        updates = 2.0 * sum(nvox * g.n_angles for nvox, _ in level_dims(g, LEVELS))
+        updates = 2.0 * sum(nvox * g.n_angles for nvox, _ in level_dims(G, LEVELS))
         print(json.dumps({"metric": METRIC, "value": whole_job_value(1, updates, args.steps, t), "unit": UNIT, "n_gpus": world,
                           "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps,
                           "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
@@ -385,6 +386,46 @@ def time_c3_recon(cb, dev, st, eq2=False):
         cb.fbs_reconstruct(G, Y, None, cfg.n_levels, [2] * cfg.n_levels, cfg.n_inner, cfg.step, cfg.mu, cfg.eps, cfg.omega, f, stream=st)
         a.record(st)
         cb.fbs_reconstruct(G, Y, None, cfg.n_levels, cfg.n_outer, cfg.n_inner, cfg.step, cfg.mu, cfg.eps, cfg.omega, f, stream=st)
+        b.record(st)
+    torch.cuda.synchronize()
+    G.close()
+    return a.elapsed_time(b) / 1e3
+
+
+def time_tv_512(cb, dev, st, flush):
+    """GB/s (12 B per voxel and sweep) of 10 TV-prox sweeps on a 512^3 volume of 0.5 mm voxels (c5's shape), L2 flushed first."""
+    import torch
+    G = cb.Geometry(1000.0, 1500.0, np.array([0.0]), 8, 8, 1.0, 1.0, 512, 512, 512, 0.5, 0.5, 0.5)
+    gv = torch.rand((512, 512, 512), device=dev) * 0.02
+    u = gv.clone()
+    best = None
+    with torch.cuda.stream(st):
+        for _ in range(4):
+            flush.fill_(1)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(st)
+            cb.tv_prox(G, gv, u, 4.0e4, 1e-4, 1.0, 10, stream=st)
+            b.record(st)
+            st.synchronize()
+            t = a.elapsed_time(b)
+            best = t if best is None else min(best, t)
+    G.close()
+    return 12.0 * 512 ** 3 * 10 / best / 1e6
+
+
+def time_c3_fdk(cb, dev, st):
+    import torch
+    from cbct_synth import make_config
+    cfg = make_config("c3")
+    g = cfg.geom
+    Y = torch.from_numpy(np.ascontiguousarray(cfg.projections(), dtype=np.float32)).to(dev)
+    G = cb.Geometry.from_synth(g)
+    f = torch.empty(g.vol_shape, device=dev)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(st):
+        cb.fdk_reconstruct(G, Y, f, stream=st)
+        a.record(st)
+        cb.fdk_reconstruct(G, Y, f, stream=st)
         b.record(st)
     torch.cuda.synchronize()
     G.close()

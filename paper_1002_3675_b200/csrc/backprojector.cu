@@ -261,6 +261,7 @@ cbct_status op_backproject_gather(cbct_geometry *g, const float *d_scaled, cudaS
 
 // out = G1 + G0^T  or  out = f - c (G1 + G0^T) [clamped]  — fuses a4 (and a6 when n_inner = 0) into the
 // transpose-add that the two-class gather needs anyway.
+template <bool PARTS>
 __global__ void __launch_bounds__(256) combine_kernel(const float *__restrict__ G0, const float *__restrict__ G1,
                                                       const float *__restrict__ f, float c, int clamp,
                                                       float *__restrict__ out, int nx, int ny, int parts, size_t nvox)
@@ -274,8 +275,11 @@ __global__ void __launch_bounds__(256) combine_kernel(const float *__restrict__ 
         for (int r = threadIdx.y; r < 32; r += 8) {
             int i = i0 + r, j = j0 + threadIdx.x;
             float v = 0.f;
-            if (i < nx && j < ny)
-                for (int p = 0; p < parts; ++p) v += __ldg(G0 + p * nvox + plane + (size_t)i * ny + j);
+            if (i < nx && j < ny) {
+                v = __ldg(G0 + plane + (size_t)i * ny + j);
+                if constexpr (PARTS)
+                    for (int p = 1; p < parts; ++p) v += __ldg(G0 + p * nvox + plane + (size_t)i * ny + j);
+            }
             tile[r][threadIdx.x] = v;
         }
         __syncthreads();
@@ -285,8 +289,11 @@ __global__ void __launch_bounds__(256) combine_kernel(const float *__restrict__ 
         if (j < ny && i < nx) {
             const size_t o = plane + (size_t)j * nx + i;
             float gsum = G0 ? tile[threadIdx.x][r] : 0.f;
-            if (G1)
-                for (int p = 0; p < parts; ++p) gsum += __ldg(G1 + p * nvox + o);
+            if (G1) {
+                gsum += __ldg(G1 + o);
+                if constexpr (PARTS)
+                    for (int p = 1; p < parts; ++p) gsum += __ldg(G1 + p * nvox + o);
+            }
             float val = gsum;
             if (f) {
                 val = fmaf(-c, gsum, __ldg(f + o));
@@ -303,7 +310,8 @@ cbct_status op_combine(cbct_geometry *g, const float *f, float c, int clamp, flo
     const float *G0 = g->n_tiles[0] > 0 ? g->G_cls[0] : nullptr;
     const float *G1 = g->n_tiles[1] > 0 ? g->G_cls[1] : nullptr;
     dim3 grid((g->nx + 31) / 32, (g->ny + 31) / 32, g->nz), block(32, 8);
-    combine_kernel<<<grid, block, 0, st>>>(G0, G1, f, c, clamp, out, g->nx, g->ny, g->bp_parts, g->n_vox());
+    if (g->bp_parts > 1) combine_kernel<true><<<grid, block, 0, st>>>(G0, G1, f, c, clamp, out, g->nx, g->ny, g->bp_parts, g->n_vox());
+    else combine_kernel<false><<<grid, block, 0, st>>>(G0, G1, f, c, clamp, out, g->nx, g->ny, 1, g->n_vox());
     CBCT_LAUNCH_CHECK();
     return CBCT_OK;
 }
