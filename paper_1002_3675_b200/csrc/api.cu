@@ -57,6 +57,13 @@ extern "C" cbct_status cbct_set_projector_staging(cbct_geometry *g, int on)
     return CBCT_OK;
 }
 
+extern "C" cbct_status cbct_set_gather_symmetry(cbct_geometry *g, int on)
+{
+    REQUIRE(g, "cbct_set_gather_symmetry: NULL handle");
+    for (cbct_geometry *q = g; q; q = q->coarse) q->bp_mirror = on != 0;
+    return CBCT_OK;
+}
+
 static float tv_dt(const cbct_geometry *g, float beta, float eps, float omega)
 {
     const double K = 4.0 * (1.0 / (g->hx * g->hx) + 1.0 / (g->hy * g->hy) + 1.0 / (g->hz * g->hz));

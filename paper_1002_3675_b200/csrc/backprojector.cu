@@ -35,6 +35,18 @@ __device__ __forceinline__ float rcp_approx(float x)
     return y;
 }
 
+// base + row * pitch (bytes): 32-bit row and pitch (either sign), 64-bit base -> one IMAD.WIDE
+__device__ __forceinline__ const char *row_ptr(const char *base, int row, int pitch) { return base + (long long)row * pitch; }
+// hides how a value was computed from the optimiser, so that an address formed from it is not re-derived from its parts
+// (ptxas would otherwise share the product row * pitch between a row and its mirror image and pay two 64-bit adds for each)
+__device__ __forceinline__ int opaque(int x) { asm("" : "+r"(x)); return x; }
+__device__ __forceinline__ const char *opaque(const char *p)
+{
+    long long x = reinterpret_cast<long long>(p);
+    asm("" : "+l"(x));
+    return reinterpret_cast<const char *>(x);
+}
+
 // C[a][v][u] = sum_{v' < v} y[a][v'][u] for v = 0..nv as (sum, compensation) pairs: the rounding
 // error of every addition is carried in the second float (two-sum), so C(v2) - C(v1) evaluated as
 // (s2 - s1) + (c2 - c1) has the accuracy of summing the run directly.
@@ -73,15 +85,20 @@ __global__ void __launch_bounds__(128) prefix_kernel(const DevGeom d, const floa
 }
 
 
-#ifndef CBCT_BP_VOTE
-#define CBCT_BP_VOTE 0
+#ifndef CBCT_BP_MINB
+#define CBCT_BP_MINB 8          // resident CTAs per SM the plain gather is compiled for (64 registers)
+#endif
+#ifndef CBCT_BP_MINB_M
+#define CBCT_BP_MINB_M 5        // the same for the mirrored gather (two accumulator columns)
 #endif
 
-#ifndef CBCT_BP_MINB
-#define CBCT_BP_MINB 8
-#endif
-template <int KC, int BI>
-__global__ void __launch_bounds__(32 * BI, CBCT_BP_MINB)
+// MIRROR: the scan is symmetric about the central plane z = 0 (nz even, detector centred in v: cv = (nv-1)/2), so ray
+// (u, nv-1-v) is the mirror image of ray (u, v) and voxel row nz-1-k that of row k.  A thread then owns a column chunk of
+// the UPPER half (planes zk >= 0) together with its mirror image: the run bounds of plane -zk are nv - vT and nv - vTn, its
+// crossing ray is nv-1-vs with the same b, and the direction of every crossing ray is the sign of dt (zeta > 0 above the
+// central plane), so the bound / crossing arithmetic of a plane (17 of its ~30 instructions) is done once for two voxel rows.
+template <int KC, int BI, bool MIRROR>
+__global__ void __launch_bounds__(32 * BI, MIRROR ? CBCT_BP_MINB_M : CBCT_BP_MINB)
 backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restrict__ angle_has,
                    const float *__restrict__ rs, const float2 *__restrict__ C, float *__restrict__ G, const int parts)
 {
@@ -91,14 +108,18 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
     // small volumes: the angle list is dealt out over `parts` CTAs per column chunk (part p takes angles p, p + parts, ...),
     // each writing its own partial volume; op_combine adds the partial volumes in the order of p
     const int kchunks = gridDim.z / parts, part = blockIdx.z / kchunks;
-    const int k0 = (blockIdx.z - part * kchunks) * KC;
+    const int k0 = (MIRROR ? d.koff : 0) + (blockIdx.z - part * kchunks) * KC;
     G += (size_t)part * d.nx * d.ny * d.nz;
     if (i >= cg.nmaj) return;                          // warp-uniform
     const bool valid = j < cg.nmin;
 
-    float acc[KC];
+    float acc[KC], accL[MIRROR ? KC : 1];
 #pragma unroll
     for (int q = 0; q < KC; ++q) acc[q] = 0.f;
+    if constexpr (MIRROR) {
+#pragma unroll
+        for (int q = 0; q < KC; ++q) accL[q] = 0.f;
+    }
 
     // the column's x-y square in mm (candidate search only; the accept test is exact)
     const float maj0 = ((float)i - 0.5f * (float)cg.nmaj) * cg.hmaj, maj1 = maj0 + cg.hmaj;
@@ -109,7 +130,8 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
     const float cu = d.cu, cv = d.cv;                  // detector index of the central ray (shifted panels: not the middle)
     const float sdd_du = d.sdd / d.du;
     const float hz_dv = d.hz / d.dv, dv_hz = d.dv / d.hz;
-    const float zk0 = (float)(k0 - d.koff) - d.zfrac;  // plane k0 in the units of z_entry(), minus zfrac
+    const int npitchC = opaque(-d.nu * (int)sizeof(float2)), npitchR = opaque(-d.nu * (int)sizeof(float));   // MIRROR: rows counted down
+    const float zk0 = (float)(k0 - d.koff) - d.zfrac;  // plane k0 in the units of z_entry(), minus zfrac (MIRROR: >= 0, an integer)
 
     for (int a = part; a < d.na; a += parts) {
         if (!angle_has[a]) continue;                   // uniform
@@ -154,10 +176,13 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
             const bool inside = fminf(fminf(fmaf(zk0, cT, cv), fmaf(zk0, cTn, cv)), fminf(fmaf(zk0 + (float)KC, cT, cv), fmaf(zk0 + (float)KC, cTn, cv))) >= 0.f &&
                                 fmaxf(fmaxf(fmaf(zk0, cT, cv), fmaf(zk0, cTn, cv)), fmaxf(fmaf(zk0 + (float)KC, cT, cv), fmaf(zk0 + (float)KC, cTn, cv))) <= (float)(d.nv - 1);
             const float xT0 = fmaf(zk0, cT, cv), xTn0 = fmaf(zk0, cTn, cv);          // bounds of plane k0; plane k0+q: + q cT (q a literal)
+            // MIRROR: prefix row nv and projection row nv-1 of this (a, u): the mirrored bound nv - vT and ray nv-1-vs are one
+            // IMAD.WIDE with the negated pitch away
+            const char *CuT = opaque(Cu + (long long)d.nv * pitchC), *RuT = opaque(Ru + (long long)(d.nv - 1) * pitchR);
+            const int up_sign = __float_as_int(dtdv) & 0x80000000;                     // MIRROR: rising iff dt > 0
             auto planes = [&](auto multi_tag, auto clamp_tag) {
                 constexpr bool MULTI = decltype(multi_tag)::value, CLAMP = decltype(clamp_tag)::value;
-                float2 c1 = make_float2(0.f, 0.f);
-                float carry = 0.f;                     // moved into the row above by the rays crossing its lower plane
+                float2 c1 = make_float2(0.f, 0.f), c1L = make_float2(0.f, 0.f);
 #pragma unroll
                 for (int q = 0; q <= KC; ++q) {
                     // first ray at or above plane k0+q at the slab's entry / exit plane
@@ -167,39 +192,54 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
                         vT = min(max(vT, 0), d.nv);
                         vTn = min(max(vTn, 0), d.nv);
                     }
-                    const float2 c2 = __ldg(reinterpret_cast<const float2 *>(Cu + (long long)vT * pitchC));
+                    const float2 c2 = __ldg(reinterpret_cast<const float2 *>(row_ptr(Cu, vT, pitchC)));
                     // rays crossing plane k0+q inside the slab: v in [min(vT,vTn), max(vT,vTn)) (y = 0 stands in if there is none).
                     // b = lambda at which the ray meets the plane: T(lambda) zeta(v) = zk with T(lambda) = T + lambda dt and
                     // zeta(v) = (v - cv) dv / hz, i.e. b = (zk - T zeta(v)) / (dt zeta(v)), the projector's b with its numerator
                     // taken by one FMA (a ray in the central plane, v = cv, crosses nothing; saturation turns its 0/0 into 0).
-                    // Only ~5 % of the (lane, plane) pairs have such a ray.  The lanes of a warp are adjacent minor rows of ONE
-                    // slab, so their ray depths T and with them their bounds are nearly equal and the crossings cluster: the warp
-                    // skips the crossing arithmetic (17 of the 31 instructions of a plane) when none of its converged lanes has one.
-                    float up = 0.f;                    // moved up across the plane (negative: moved down)
-                    if (!CBCT_BP_VOTE || __any_sync(__activemask(), vT != vTn)) {
-                        const int dlt = vTn - vT, vs = min(vT, vTn);
-                        const float vf = (float)vs - cv;
-                        const float bq = __saturatef(fmaf(-Tdv, vf, zk) * rcp_approx(vf * dtdv));
-                        // rising iff dt zeta(v) > 0: move the sign bit of dt zeta(v) onto y
-                        float yq = 0.f;
-                        if (dlt != 0) yq = __ldg(reinterpret_cast<const float *>(Ru + (long long)vs * pitchR));
-                        yq = __int_as_float(__float_as_int(yq) ^ (__float_as_int(vf * dtdv) & 0x80000000));
-                        up = fmaxf(0.f, l1 - fmaxf(l0, bq)) * yq;
-                        if constexpr (MULTI) {
-                            for (int v = vs + 1; v < vs + abs(dlt); ++v) {   // further rays crossing this plane (fine detector rows)
-                                const float vf2 = (float)v - cv;
-                                const float b2 = __saturatef(fmaf(-Tdv, vf2, zk) * rcp_approx(vf2 * dtdv));
-                                const float y2 = __ldg(reinterpret_cast<const float *>(Ru + (long long)v * pitchR));
-                                up = fmaf(fmaxf(0.f, l1 - fmaxf(l0, b2)), __int_as_float(__float_as_int(y2) ^ (__float_as_int(vf * dtdv) & 0x80000000)), up);
-                            }
+                    const int dlt = vTn - vT, vs = min(vT, vTn);
+                    const float vf = (float)vs - cv;
+                    const float bq = __saturatef(fmaf(-Tdv, vf, zk) * rcp_approx(vf * dtdv));
+                    // fraction of the ray's chord in this row that lies beyond the plane, signed: positive = it rises across the
+                    // plane (dt zeta(v) > 0), so the fraction moves from the row below the plane to the row above it
+                    const int sgn = MIRROR ? up_sign : (__float_as_int(vf * dtdv) & 0x80000000);
+                    const float fs = __int_as_float(__float_as_int(fmaxf(0.f, l1 - fmaxf(l0, bq))) ^ sgn);
+                    float yq = 0.f;
+                    if (dlt != 0) yq = __ldg(reinterpret_cast<const float *>(row_ptr(Ru, vs, pitchR)));
+                    float up = fs * yq;                // moved up across the plane (negative: moved down)
+                    // the mirror image: plane -zk, bounds nv - vT (plane 0 is its own image: the same bound, so that a ray lying
+                    // in it belongs to the row above it on both sides), crossing ray nv-1-vs, rising <-> falling
+                    [[maybe_unused]] float2 c2L;
+                    [[maybe_unused]] float dn = 0.f;                    // moved DOWN across the mirrored plane
+                    if constexpr (MIRROR) {
+                        c2L = (q == 0 && zk0 == 0.f) ? c2 : __ldg(reinterpret_cast<const float2 *>(row_ptr(CuT, vT, npitchC)));
+                        float yL = 0.f;
+                        if (dlt != 0) yL = __ldg(reinterpret_cast<const float *>(row_ptr(RuT, vs, npitchR)));
+                        dn = fs * yL;
+                    }
+                    if constexpr (MULTI) {
+                        for (int v = vs + 1; v < vs + abs(dlt); ++v) {   // further rays crossing this plane (fine detector rows)
+                            const float vf2 = (float)v - cv;
+                            const float b2 = __saturatef(fmaf(-Tdv, vf2, zk) * rcp_approx(vf2 * dtdv));
+                            const float f2 = __int_as_float(__float_as_int(fmaxf(0.f, l1 - fmaxf(l0, b2))) ^ sgn);
+                            up = fmaf(f2, __ldg(reinterpret_cast<const float *>(row_ptr(Ru, v, pitchR))), up);
+                            if constexpr (MIRROR) dn = fmaf(f2, __ldg(reinterpret_cast<const float *>(row_ptr(RuT, v, npitchR))), dn);
                         }
                     }
                     if (q > 0) {
                         const float ysum = (c2.x - c1.x) + (c2.y - c1.y);
-                        acc[q > 0 ? q - 1 : 0] += fmaf(w, ysum, carry - up);
+                        acc[q > 0 ? q - 1 : 0] = fmaf(w, ysum, acc[q > 0 ? q - 1 : 0]) - up;
+                        if constexpr (MIRROR) {
+                            const float ysumL = (c1L.x - c2L.x) + (c1L.y - c2L.y);
+                            accL[q > 0 ? q - 1 : 0] = fmaf(w, ysumL, accL[q > 0 ? q - 1 : 0]) - dn;
+                        }
+                    }
+                    if (q < KC) {
+                        acc[q < KC ? q : 0] += up;
+                        if constexpr (MIRROR) accL[q < KC ? q : 0] += dn;
                     }
                     c1 = c2;
-                    carry = up;
+                    if constexpr (MIRROR) c1L = c2L;
                 }
             };
             if (single && inside) planes(std::false_type{}, std::false_type{});
@@ -211,7 +251,10 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
 #pragma unroll
     for (int q = 0; q < KC; ++q) {
         const int k = k0 + q;
-        if (k < d.nz) G[((size_t)k * cg.nmaj + i) * cg.nmin + j] = acc[q];
+        if (k < d.nz) {
+            G[((size_t)k * cg.nmaj + i) * cg.nmin + j] = acc[q];
+            if constexpr (MIRROR) G[((size_t)(d.nz - 1 - k) * cg.nmaj + i) * cg.nmin + j] = accL[q];
+        }
     }
 }
 
@@ -225,23 +268,19 @@ cbct_status op_backproject_prefix(cbct_geometry *g, const float *d_in, int scale
     return CBCT_OK;
 }
 
-cbct_status op_backproject_gather(cbct_geometry *g, const float *d_scaled, cudaStream_t st)
+template <int KC, int BI, bool MIRROR>
+static cbct_status launch_gather(cbct_geometry *g, const float *d_scaled, cudaStream_t st)
 {
-    // z rows per thread and slabs per CTA: compile-time tuning knobs (measured best of a sweep on B200: 16 x 4)
-#ifndef CBCT_BP_KC
-#define CBCT_BP_KC 16
-#define CBCT_BP_BI 4
-#endif
-    constexpr int KC = CBCT_BP_KC, BI = CBCT_BP_BI;
-    ProfileScope ps(3, st);
     // A small volume has too few voxel columns to fill the GPU (c1: 16 CTAs per class, 70 us per launch whatever the clock):
     // the angles are then dealt out over up to 8 CTAs per column chunk, aiming at two CTAs per SM
+    const int rows = MIRROR ? g->nz / 2 : g->nz;       // voxel rows the chunks cover (MIRROR: the upper half)
+    const int kchunks = (rows + KC - 1) / KC;
     g->bp_parts = 1;
     {
         int dev = 0, sms = 148;
         if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         const ClassGrid &cg = g->dev.cls[0];
-        const long ctas = (long)((cg.nmin + 31) / 32) * ((cg.nmaj + BI - 1) / BI) * ((g->nz + KC - 1) / KC);
+        const long ctas = (long)((cg.nmin + 31) / 32) * ((cg.nmaj + BI - 1) / BI) * kchunks;
         while (g->bp_parts < 8 && ctas * g->bp_parts < 2L * sms && 2 * g->bp_parts <= g->na) g->bp_parts *= 2;
     }
     for (int c = 0; c < 2; ++c) {
@@ -252,11 +291,32 @@ cbct_status op_backproject_gather(cbct_geometry *g, const float *d_scaled, cudaS
             g->G_parts_alloc[c] = g->bp_parts;
         }
         const ClassGrid &cg = g->dev.cls[c];
-        dim3 grid((cg.nmin + 31) / 32, (cg.nmaj + BI - 1) / BI, ((g->nz + KC - 1) / KC) * g->bp_parts), block(32, BI);
-        backproject_kernel<KC, BI><<<grid, block, 0, st>>>(g->dev, c, g->d_angle_has[c], d_scaled, g->proj_prefix, g->G_cls[c], g->bp_parts);
+        dim3 grid((cg.nmin + 31) / 32, (cg.nmaj + BI - 1) / BI, kchunks * g->bp_parts), block(32, BI);
+        backproject_kernel<KC, BI, MIRROR><<<grid, block, 0, st>>>(g->dev, c, g->d_angle_has[c], d_scaled, g->proj_prefix, g->G_cls[c], g->bp_parts);
         CBCT_LAUNCH_CHECK();
     }
     return CBCT_OK;
+}
+
+// the scan is its own mirror image about the central plane: an even number of slices and a detector centred in v
+bool gather_is_mirrored(const cbct_geometry *g)
+{
+    return g->bp_mirror && g->nz % 2 == 0 && g->off_v == 0.0;
+}
+
+cbct_status op_backproject_gather(cbct_geometry *g, const float *d_scaled, cudaStream_t st)
+{
+    // z rows per thread and slabs per CTA: compile-time tuning knobs (measured best of a sweep on B200)
+#ifndef CBCT_BP_KC
+#define CBCT_BP_KC 16
+#define CBCT_BP_BI 4
+#endif
+#ifndef CBCT_BP_KC_M
+#define CBCT_BP_KC_M 16
+#endif
+    ProfileScope ps(3, st);
+    if (gather_is_mirrored(g)) return launch_gather<CBCT_BP_KC_M, CBCT_BP_BI, true>(g, d_scaled, st);
+    return launch_gather<CBCT_BP_KC, CBCT_BP_BI, false>(g, d_scaled, st);
 }
 
 // out = G1 + G0^T  or  out = f - c (G1 + G0^T) [clamped]  — fuses a4 (and a6 when n_inner = 0) into the

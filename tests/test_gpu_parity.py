@@ -138,6 +138,29 @@ def test_tma_staged_projector_equals_the_cached_march(cuda_lib, dev, name):
     G0.close(); G1.close()
 
 
+@pytest.mark.parametrize("name", ["c1", "aniso_ragged", "wide_detector_misses", "short_arc_200deg", "fine_rows_multicross", "fine_columns",
+                                  "coarse_detector", "one_column", "odd_rows_even_slices", "odd_rows_even_slices_coarse"])
+def test_plain_gather_equals_the_mirrored_gather(cuda_lib, dev, name):
+    """Scans that are their own mirror image about z = 0 (nz even, detector centred in v) are gathered two voxel rows at a
+    time (cbct_set_gather_symmetry, the default); the plain gather (forced here, and the only one for odd nz or shifted
+    panels) must give the same transpose: both within the operator tolerance of the oracle, and equal to each other to
+    fp32 summation order, on phantom-like projections and on Gaussian ones."""
+    cb = cuda_lib
+    g = GEOMS[name]()
+    assert g.nz % 2 == 0
+    G = cb.Geometry.from_synth(g)
+    vol = f32(smooth_phantom(g, 5) if name != "c1" else make_config("c1").volume())
+    for y, tol in ((run_forward(cb, G, vol, dev), TOL_OP), (f32(gaussian_field(g.proj_shape, 21)), 5e-5)):
+        ref = o.backproject(g, y.astype(np.float64))
+        G.set_gather_symmetry(True)
+        b_m = run_backproject(cb, G, y, dev)
+        G.set_gather_symmetry(False)
+        b_p = run_backproject(cb, G, y, dev)
+        assert rel(b_m, ref) <= tol and rel(b_p, ref) <= tol
+        assert rel(b_m, b_p.astype(np.float64)) <= 2e-6
+    G.close()
+
+
 def test_backproject_of_unit_projections_matches_brute_force_clip(cuda_lib, dev):
     """Exact adjoint, entry by entry: P^T applied to single-pixel images equals the matrix column
     the oracle gets by clipping that ray against each voxel box."""
