@@ -47,6 +47,13 @@ __device__ __forceinline__ const char *opaque(const char *p)
     return reinterpret_cast<const char *>(x);
 }
 
+// a + b = s + two_sum_err(a, b, s) exactly, for s = fl(a + b) (Knuth's two-sum; no assumption on the magnitudes)
+__device__ __forceinline__ float two_sum_err(float a, float b, float s)
+{
+    const float bb = __fsub_rn(s, a);
+    return __fadd_rn(__fsub_rn(a, __fsub_rn(s, bb)), __fsub_rn(b, bb));
+}
+
 // C[a][v][u] = sum_{v' < v} y[a][v'][u] for v = 0..nv as (sum, compensation) pairs: the rounding
 // error of every addition is carried in the second float (two-sum), so C(v2) - C(v1) evaluated as
 // (s2 - s1) + (c2 - c1) has the accuracy of summing the run directly.
@@ -129,8 +136,8 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
     const float ef = (float)(i - cg.ioff);
     const float cu = d.cu, cv = d.cv;                  // detector index of the central ray (shifted panels: not the middle)
     const float sdd_du = d.sdd / d.du;
-    const float hz_dv = d.hz / d.dv, dv_hz = d.dv / d.hz;
     const int npitchC = opaque(-d.nu * (int)sizeof(float2)), npitchR = opaque(-d.nu * (int)sizeof(float));   // MIRROR: rows counted down
+    const float inv_hzdv = rcp_approx(d.hzdv_hi);
     const float zk0 = (float)(k0 - d.koff) - d.zfrac;  // plane k0 in the units of z_entry(), minus zfrac (MIRROR: >= 0, an integer)
 
     for (int a = part; a < d.na; a += parts) {
@@ -161,32 +168,54 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
             const float w = l1 - l0;
             if (!(w > 0.f)) continue;
 
-            const float T = fmaf(ef, r.dt, r.tc), Tn = fmaf(ef + 1.f, r.dt, r.tc);   // entry / exit ray parameter
-            const float cT = hz_dv * rcp_approx(T), cTn = hz_dv * rcp_approx(Tn);     // d v / d z at entry / exit (T > 0)
+            // Entry ray parameter T = tc + ef dt and the detector rows per z plane at the entry plane, cT = (hz / dv) / T, as
+            // unevaluated sums of two floats: a z plane zk meets the detector at row cv + zk cT, |zk cT| up to several hundred
+            // rows, and the crossing fraction of a ray amplifies an error in that position by (T / dt) / |v - cv| (4 at c5):
+            // plain fp32 leaves 1e-4 of a chord there.  The exit plane only detects crossings; fp32 is enough for it.
+            // (__fmul_rn / __fadd_rn / __fsub_rn are never contracted into FMAs, which would break the error-free sums)
+            const float p_hi = __fmul_rn(ef, r.dt), p_lo = fmaf(ef, r.dt, -p_hi);
+            const float T = __fadd_rn(r.tc, p_hi);
+            const float T_lo = two_sum_err(r.tc, p_hi, T) + p_lo;
+            const float Tn = fmaf(ef + 1.f, r.dt, r.tc);
+            const float rT = rcp_approx(T);
+            const float cT = __fmul_rn(d.hzdv_hi, rT), cTn = d.hzdv_hi * rcp_approx(Tn);          // d v / d z at entry / exit (T > 0)
+            // rho = (true cT - cT) / cT from the exact remainder hz/dv - cT (T + T_lo)
+            const float rho = __fadd_rn(fmaf(-cT, T_lo, fmaf(-cT, T, d.hzdv_hi)), d.hzdv_lo) * inv_hzdv;
             // 32-bit element offsets of (a, v = 0, u) in the prefix sums and in the projections (checked at geometry creation)
             // byte offsets: one IMAD.WIDE (row * pitch + base) forms the address of a row's element
             const char *Cu = reinterpret_cast<const char *>(C + (a * (d.nv + 1) * d.nu + u));
             const char *Ru = reinterpret_cast<const char *>(rs + (a * d.nv * d.nu + u));
             const int pitchC = d.nu * (int)sizeof(float2), pitchR = d.nu * (int)sizeof(float);
-            const float Tdv = T * dv_hz, dtdv = r.dt * dv_hz;                         // T zeta(v) = Tdv (v - cv), dt zeta(v) = dtdv (v - cv)
+            // b = lambda at which ray v meets plane zk: (T + b dt) (v - cv) dv / hz = zk.  With delta = (v - cv) - zk cT, the
+            // distance of the ray from where the plane meets the detector at the slab's entry, b = -(T / dt) delta / (v - cv).
+            const float TD = T * r.inv_dt;
+            const float l1c = fmaf(-TD, rho, l1);
             // entry and exit bounds of a plane less than one detector row apart on every plane of the chunk: at most one
             // ray crosses a plane inside the slab, and the loop over further crossing rays is compiled out
             const bool single = fmaxf(fabsf(zk0), fabsf(zk0 + (float)KC)) * fabsf(cT - cTn) < 0.999f;
-            // all run bounds of the chunk fall on the detector: no clamping needed
-            const bool inside = fminf(fminf(fmaf(zk0, cT, cv), fmaf(zk0, cTn, cv)), fminf(fmaf(zk0 + (float)KC, cT, cv), fmaf(zk0 + (float)KC, cTn, cv))) >= 0.f &&
-                                fmaxf(fmaxf(fmaf(zk0, cT, cv), fmaf(zk0, cTn, cv)), fmaxf(fmaf(zk0 + (float)KC, cT, cv), fmaf(zk0 + (float)KC, cTn, cv))) <= (float)(d.nv - 1);
-            const float xT0 = fmaf(zk0, cT, cv), xTn0 = fmaf(zk0, cTn, cv);          // bounds of plane k0; plane k0+q: + q cT (q a literal)
+            // all run bounds of the chunk fall on the detector: no clamping needed (MIRROR: zk >= 0, so the bounds lie between cv
+            // and the top plane's, and their mirror images do the same below)
+            bool inside;
+            if constexpr (MIRROR) inside = fmaf(zk0 + (float)KC, fmaxf(cT, cTn), cv) <= (float)(d.nv - 1);
+            else inside = fminf(fminf(fmaf(zk0, cT, cv), fmaf(zk0, cTn, cv)), fminf(fmaf(zk0 + (float)KC, cT, cv), fmaf(zk0 + (float)KC, cTn, cv))) >= 0.f &&
+                          fmaxf(fmaxf(fmaf(zk0, cT, cv), fmaf(zk0, cTn, cv)), fmaxf(fmaf(zk0 + (float)KC, cT, cv), fmaf(zk0 + (float)KC, cTn, cv))) <= (float)(d.nv - 1);
+            // bounds of plane k0 (plane k0+q: + q cT, q a literal); the entry bound as xT0 + x_lo, x_lo = what the float drops of
+            // cv + zk0 cT (exact product by FMA, exact sum by two-sum).  The plane really sits at cv + zk cT (1 + rho): with
+            // delta' = (v - cv) - zk cT, delta = delta' - rho zk cT = delta' - rho (v - cv) to first order, so
+            // l1 - b = (l1 - (T / dt) rho) + (T / dt) delta' / (v - cv): the correction costs nothing per plane.
+            const float P_hi = __fmul_rn(zk0, cT), P_lo = fmaf(zk0, cT, -P_hi);
+            const float xT0 = __fadd_rn(cv, P_hi), xTn0 = fmaf(zk0, cTn, cv);
+            const float x_lo = (two_sum_err(cv, P_hi, xT0) + P_lo) + d.cv_lo;
             // MIRROR: prefix row nv and projection row nv-1 of this (a, u): the mirrored bound nv - vT and ray nv-1-vs are one
             // IMAD.WIDE with the negated pitch away
             const char *CuT = opaque(Cu + (long long)d.nv * pitchC), *RuT = opaque(Ru + (long long)(d.nv - 1) * pitchR);
-            const int up_sign = __float_as_int(dtdv) & 0x80000000;                     // MIRROR: rising iff dt > 0
+            const int up_sign = __float_as_int(r.dt) & 0x80000000;                     // MIRROR: rising iff dt > 0
             auto planes = [&](auto multi_tag, auto clamp_tag) {
                 constexpr bool MULTI = decltype(multi_tag)::value, CLAMP = decltype(clamp_tag)::value;
                 float2 c1 = make_float2(0.f, 0.f), c1L = make_float2(0.f, 0.f);
 #pragma unroll
                 for (int q = 0; q <= KC; ++q) {
                     // first ray at or above plane k0+q at the slab's entry / exit plane
-                    const float zk = zk0 + (float)q;
                     int vT = (int)ceilf(fmaf((float)q, cT, xT0)), vTn = (int)ceilf(fmaf((float)q, cTn, xTn0));
                     if constexpr (CLAMP) {
                         vT = min(max(vT, 0), d.nv);
@@ -194,16 +223,20 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
                     }
                     const float2 c2 = __ldg(reinterpret_cast<const float2 *>(row_ptr(Cu, vT, pitchC)));
                     // rays crossing plane k0+q inside the slab: v in [min(vT,vTn), max(vT,vTn)) (y = 0 stands in if there is none).
-                    // b = lambda at which the ray meets the plane: T(lambda) zeta(v) = zk with T(lambda) = T + lambda dt and
-                    // zeta(v) = (v - cv) dv / hz, i.e. b = (zk - T zeta(v)) / (dt zeta(v)), the projector's b with its numerator
-                    // taken by one FMA (a ray in the central plane, v = cv, crosses nothing; saturation turns its 0/0 into 0).
+                    // The part of such a ray's chord in this minor row that lies beyond the plane is
+                    //   max(0, l1 - max(l0, sat(b))) = min(sat(l1 - b), l1 - l0)       (0 <= l0 <= l1 <= 1)
+                    // — its exit-row fraction among the projector's four.  A ray in the central plane (v = cv, only met at zk = 0)
+                    // crosses nothing: its 0 * inf is a NaN that the saturation turns into 0.
                     const int dlt = vTn - vT, vs = min(vT, vTn);
-                    const float vf = (float)vs - cv;
-                    const float bq = __saturatef(fmaf(-Tdv, vf, zk) * rcp_approx(vf * dtdv));
-                    // fraction of the ray's chord in this row that lies beyond the plane, signed: positive = it rises across the
-                    // plane (dt zeta(v) > 0), so the fraction moves from the row below the plane to the row above it
-                    const int sgn = MIRROR ? up_sign : (__float_as_int(vf * dtdv) & 0x80000000);
-                    const float fs = __int_as_float(__float_as_int(fmaxf(0.f, l1 - fmaxf(l0, bq))) ^ sgn);
+                    const float vsf = (float)vs, vf = vsf - cv;
+                    // delta = vs - (cv + (zk0 + q) cT): vs - xT0 is exact (both below 2^11 and a few rows apart), the FMA rounds a
+                    // number of a few rows at most, x_lo restores what xT0 dropped
+                    const float dl = __fsub_rn(fmaf(-(float)q, cT, __fsub_rn(vsf, xT0)), x_lo);
+                    const float fr = fminf(__saturatef(fmaf(TD, dl * rcp_approx(vf), l1c)), w);
+                    // signed: positive = the ray rises across the plane (dt zeta(v) > 0), so the fraction moves from the row below
+                    // the plane to the row above it
+                    const int sgn = MIRROR ? up_sign : ((__float_as_int(vf) ^ __float_as_int(r.dt)) & 0x80000000);
+                    const float fs = __int_as_float(__float_as_int(fr) ^ sgn);
                     float yq = 0.f;
                     if (dlt != 0) yq = __ldg(reinterpret_cast<const float *>(row_ptr(Ru, vs, pitchR)));
                     float up = fs * yq;                // moved up across the plane (negative: moved down)
@@ -219,9 +252,9 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
                     }
                     if constexpr (MULTI) {
                         for (int v = vs + 1; v < vs + abs(dlt); ++v) {   // further rays crossing this plane (fine detector rows)
-                            const float vf2 = (float)v - cv;
-                            const float b2 = __saturatef(fmaf(-Tdv, vf2, zk) * rcp_approx(vf2 * dtdv));
-                            const float f2 = __int_as_float(__float_as_int(fmaxf(0.f, l1 - fmaxf(l0, b2))) ^ sgn);
+                            const float dl2 = __fsub_rn(fmaf(-(float)q, cT, __fsub_rn((float)v, xT0)), x_lo);
+                            const float fr2 = fminf(__saturatef(fmaf(TD, dl2 * rcp_approx((float)v - cv), l1c)), w);
+                            const float f2 = __int_as_float(__float_as_int(fr2) ^ sgn);
                             up = fmaf(f2, __ldg(reinterpret_cast<const float *>(row_ptr(Ru, v, pitchR))), up);
                             if constexpr (MIRROR) dn = fmaf(f2, __ldg(reinterpret_cast<const float *>(row_ptr(RuT, v, npitchR))), dn);
                         }

@@ -50,6 +50,8 @@ struct DevGeom {
     float zfrac;                // nz/2.0 - koff  (0 or 0.5)
     float hx, hy, hz, du, dv, sad, sdd;
     float cu, cv;               // detector index of the central ray: (nu-1)/2 - off_u/du, (nv-1)/2 - off_v/dv
+    float cv_lo;                // the part of that v index the float cv drops (0 for a centred panel)
+    float hzdv_hi, hzdv_lo;     // hz / dv as an unevaluated sum of two floats (the gather places z planes on the detector with it)
     ClassGrid cls[2];
     const RayXY *rays;          // [na][nu]
     const float *zeta;          // [nv]  Dz(v)/hz

@@ -93,6 +93,9 @@ static cbct_status build_tables(cbct_geometry *g)
     d.du = (float)g->du; d.dv = (float)g->dv; d.sad = (float)g->sad; d.sdd = (float)g->sdd;
     d.cu = (float)(0.5 * (nu - 1) - g->off_u / g->du);
     d.cv = (float)(0.5 * (nv - 1) - g->off_v / g->dv);
+    d.cv_lo = (float)((0.5 * (nv - 1) - g->off_v / g->dv) - (double)d.cv);
+    d.hzdv_hi = (float)(g->hz / g->dv);
+    d.hzdv_lo = (float)(g->hz / g->dv - (double)d.hzdv_hi);
     for (int c = 0; c < 2; ++c) {
         ClassGrid &cg = d.cls[c];
         cg.nmaj = c == 0 ? g->nx : g->ny;
