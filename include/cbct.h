@@ -124,13 +124,14 @@ cbct_status cbct_set_projector_staging(cbct_geometry *g, int on);
 cbct_status cbct_backproject(const cbct_geometry *g, const float *d_proj, float *d_vol, void *cuda_stream);
 
 /*
- * Whether cbct_backproject (and step 1 of A1) may use the scan's mirror symmetry about the central plane z = 0: on = 1 (the
- * default) lets a thread gather a voxel row and its mirror image nz-1-k from one evaluation of the run bounds and crossing
- * fractions wherever the geometry is its own mirror image (nz even, no detector shift in v); on = 0 forces the plain gather.
- * Same matrix entries either way (the mirrored ray (u, nv-1-v) has the mirrored chords, O1); results equal to fp32 rounding.
- * Applies to this handle and its coarse levels.
+ * Whether the projector and the exact backprojector may use the scan's mirror symmetry about the central plane z = 0: on = 1
+ * (the default) lets a thread march ray (u, v) together with its mirror image (u, nv-1-v), and gather a voxel row k together
+ * with its mirror image nz-1-k, from one evaluation of the z arithmetic, wherever the geometry is its own mirror image (nz
+ * even, no detector shift in v; the projector also needs nv even); on = 0 forces the plain kernels.  Same matrix entries
+ * either way (the mirrored ray has the mirrored chords, O1); results equal to fp32 rounding.  Applies to this handle and its
+ * coarse levels.
  */
-cbct_status cbct_set_gather_symmetry(cbct_geometry *g, int on);
+cbct_status cbct_set_mirror_symmetry(cbct_geometry *g, int on);
 
 /*
  * NEXT-1. The paper's own voxel-driven backprojector, eq. 2, without its prefactor 2/(N_theta A):

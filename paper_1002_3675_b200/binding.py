@@ -15,7 +15,7 @@ STATUS = {0: "CBCT_OK", 1: "CBCT_ERR_INVALID_ARG", 2: "CBCT_ERR_SHAPE", 3: "CBCT
 # every symbol include/cbct.h declares (tests check that the library exports each of them)
 SYMBOLS = (
     "cbct_geometry_create", "cbct_geometry_create_ex", "cbct_set_detector_binning", "cbct_fbs_vcycle", "cbct_fdk_reconstruct",
-    "cbct_fbs_reconstruct_sharded", "cbct_cascade_run", "cbct_set_projector_staging", "cbct_set_gather_symmetry", "cbct_geometry_destroy", "cbct_geometry_query", "cbct_geometry_coarsen",
+    "cbct_fbs_reconstruct_sharded", "cbct_cascade_run", "cbct_set_projector_staging", "cbct_set_mirror_symmetry", "cbct_geometry_destroy", "cbct_geometry_query", "cbct_geometry_coarsen",
     "cbct_forward", "cbct_backproject", "cbct_backproject_eq2", "cbct_set_backprojector", "cbct_tv_prox", "cbct_prolong", "cbct_restrict", "cbct_bin2x2",
     "cbct_energy", "cbct_data_gradient", "cbct_prox_step", "cbct_fbs_reconstruct", "cbct_fbs_reconstruct_until", "cbct_forward_host", "cbct_backproject_host", "cbct_tv_prox_host",
     "cbct_fbs_reconstruct_host", "cbct_profile_enable", "cbct_profile_read", "cbct_launch_count", "cbct_device_bytes", "cbct_last_error",
@@ -67,7 +67,7 @@ def load():
     L.cbct_geometry_create_ex.argtypes = [d, d, dp, i, i, i, d, d, d, d, i, i, i, d, d, d, C.POINTER(vp)]
     L.cbct_set_detector_binning.argtypes = [vp, i]
     L.cbct_set_projector_staging.argtypes = [vp, i]
-    L.cbct_set_gather_symmetry.argtypes = [vp, i]
+    L.cbct_set_mirror_symmetry.argtypes = [vp, i]
     L.cbct_fbs_vcycle.argtypes = [vp, fp, fp, i, i, i, i, i, i, f, f, f, f, fp, dp, vp]
     L.cbct_fdk_reconstruct.argtypes = [vp, fp, fp, vp]
     L.cbct_fbs_reconstruct_sharded.argtypes = [vp, fp, fp, i, ip, i, f, f, f, f, i, ALLREDUCE_FN, vp, fp, fp, vp]
@@ -221,9 +221,9 @@ class Geometry:
         """Projector fed by TMA-staged shared-memory bricks (True) or by the L1-cached march (False, default)."""
         _check(load().cbct_set_projector_staging(self._h, 1 if on else 0))
 
-    def set_gather_symmetry(self, on: bool):
-        """Exact backprojector: gather mirrored voxel rows together where the scan is symmetric about z = 0 (True, default)."""
-        _check(load().cbct_set_gather_symmetry(self._h, 1 if on else 0))
+    def set_mirror_symmetry(self, on: bool):
+        """Projector / exact backprojector: treat mirrored rays / voxel rows together where the scan is symmetric about z = 0 (True, default)."""
+        _check(load().cbct_set_mirror_symmetry(self._h, 1 if on else 0))
 
     def set_detector_binning(self, on: bool):
         """Coarse levels bin the detector 2x2 (default) or keep it at full resolution; drops existing coarse levels."""

@@ -57,10 +57,10 @@ extern "C" cbct_status cbct_set_projector_staging(cbct_geometry *g, int on)
     return CBCT_OK;
 }
 
-extern "C" cbct_status cbct_set_gather_symmetry(cbct_geometry *g, int on)
+extern "C" cbct_status cbct_set_mirror_symmetry(cbct_geometry *g, int on)
 {
-    REQUIRE(g, "cbct_set_gather_symmetry: NULL handle");
-    for (cbct_geometry *q = g; q; q = q->coarse) q->bp_mirror = on != 0;
+    REQUIRE(g, "cbct_set_mirror_symmetry: NULL handle");
+    for (cbct_geometry *q = g; q; q = q->coarse) q->use_mirror = on != 0;
     return CBCT_OK;
 }
 

@@ -216,7 +216,18 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
 #pragma unroll
                 for (int q = 0; q <= KC; ++q) {
                     // first ray at or above plane k0+q at the slab's entry / exit plane
-                    int vT = (int)ceilf(fmaf((float)q, cT, xT0)), vTn = (int)ceilf(fmaf((float)q, cTn, xTn0));
+                    // (plain gather: from zk itself, so that the central plane zk = 0 sits at cv exactly, its two bounds agree and a
+                    // ray lying in it — odd nv, even nz — crosses nothing and belongs to the row above; the mirrored gather meets that
+                    // plane only as q = 0 of the chunk with zk0 = 0, where xT0 = xTn0 = cv)
+                    int vT, vTn;
+                    if constexpr (MIRROR) {
+                        vT = (int)ceilf(fmaf((float)q, cT, xT0));
+                        vTn = (int)ceilf(fmaf((float)q, cTn, xTn0));
+                    } else {
+                        const float zk = zk0 + (float)q;
+                        vT = (int)ceilf(fmaf(zk, cT, cv));
+                        vTn = (int)ceilf(fmaf(zk, cTn, cv));
+                    }
                     if constexpr (CLAMP) {
                         vT = min(max(vT, 0), d.nv);
                         vTn = min(max(vTn, 0), d.nv);
@@ -334,7 +345,7 @@ static cbct_status launch_gather(cbct_geometry *g, const float *d_scaled, cudaSt
 // the scan is its own mirror image about the central plane: an even number of slices and a detector centred in v
 bool gather_is_mirrored(const cbct_geometry *g)
 {
-    return g->bp_mirror && g->nz % 2 == 0 && g->off_v == 0.0;
+    return g->use_mirror && g->nz % 2 == 0 && g->off_v == 0.0;
 }
 
 cbct_status op_backproject_gather(cbct_geometry *g, const float *d_scaled, cudaStream_t st)

@@ -96,7 +96,7 @@ struct cbct_geometry {
 
     int bp_parts = 1, G_parts_alloc[2] = {0, 0};   // gather: angle parts per column chunk (small volumes), partial volumes allocated
     int bp_mode = 0;                          // step 1 of A1: 0 exact transpose, 1 eq. 2 (cbct_set_backprojector)
-    int bp_mirror = 1;                        // gather: use the scan's mirror symmetry about z = 0 where it has one (cbct_set_gather_symmetry)
+    int use_mirror = 1;                        // march and gather: use the scan's mirror symmetry about z = 0 where it has one (cbct_set_mirror_symmetry)
     int fw_staged = 0;                        // projector: 1 = TMA-staged bricks (projector_tma.cu), 0 = __ldg march
     int fw_bj[2] = {0, 0}, fw_bk[2] = {0, 0};  // brick spans per class (0 = not computed yet)
     int bin_detector = 1;                     // coarse levels bin the detector 2x2 (O6) or keep it at full resolution (Q20)

@@ -320,7 +320,7 @@ extern "C" cbct_status cbct_geometry_coarsen(const cbct_geometry *gc, cbct_geome
         c->bp_mode = g->bp_mode;
         c->bin_detector = g->bin_detector;
         c->fw_staged = g->fw_staged;
-        c->bp_mirror = g->bp_mirror;
+        c->use_mirror = g->use_mirror;
         g->coarse = c;
         std::memcpy(g->coarsen_flags, fl, sizeof(fl));
     }

@@ -59,7 +59,11 @@ cbct_status op_pad_copies(cbct_geometry *g, const float *d_vol, cudaStream_t st)
 // ------------------------------------------------------------------------------------------
 // Forward march.
 // ------------------------------------------------------------------------------------------
-template <int V, int WARPS>
+// MIRROR: the scan is its own mirror image about the central plane z = 0 (nz even, nv even, detector centred in v).  Ray
+// (u, nv-1-v) is then the mirror image of ray (u, v): same x-y traversal, same crossing positions b, z rows nz-1-k.  A thread
+// marches V rays of the UPPER half of the detector (v >= nv/2) together with their V mirror images, so the z arithmetic of a
+// slab (entry position, b, the row advance and its clamps) is done once for two rays.
+template <int V, int WARPS, bool MIRROR>
 __global__ void __launch_bounds__(32 * WARPS)
 forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, const float *__restrict__ vol,
                float *__restrict__ out, const float *__restrict__ Y, const int mode)
@@ -68,7 +72,8 @@ forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, c
     const int lane = threadIdx.x;
     const int2 tile = tiles[blockIdx.x];
     const int a = tile.x, u = tile.y + lane;
-    const int v0 = (blockIdx.y * WARPS + threadIdx.y) * V;
+    const int vbase = MIRROR ? d.nv / 2 : 0;                  // first detector row this launch marches directly
+    const int v0 = vbase + (blockIdx.y * WARPS + threadIdx.y) * V;
     if (v0 >= d.nv) return;                                   // warp-uniform
 
     RayXY r = load_ray(d, a, min(u, d.nu - 1));
@@ -93,9 +98,13 @@ forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, c
     const int lo_w = __reduce_min_sync(0xffffffffu, active ? ilo : 0x7fffffff);
     const int hi_w = __reduce_max_sync(0xffffffffu, active ? ihi : -1);
 
-    float acc[V];
+    float acc[V], accM[MIRROR ? V : 1];
 #pragma unroll
     for (int q = 0; q < V; ++q) acc[q] = 0.f;
+    if constexpr (MIRROR) {
+#pragma unroll
+        for (int q = 0; q < V; ++q) accM[q] = 0.f;
+    }
 
     if (lo_w < hi_w) {
         const float dirpos = r.sm >= 0.f ? 1.f : 0.f;
@@ -103,6 +112,8 @@ forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, c
         float zeta[V], inv_sz[V], zbnd[V];
         int krow[V], rowoff[V];                                          // element offsets fit 32 bits (checked at geometry creation)
         const int pstride = (int)cg.plane_stride;
+        // MIRROR: padded row of the mirror image = (nz - 1 + 2 kPadK) - padded row (the clamp range is symmetric)
+        const int row_top = (d.nz - 1 + 2 * kPadK) * pstride;
         const float e0 = (float)(lo_w - cg.ioff);
         const float T0 = fmaf(e0, r.dt, r.tc);
 #pragma unroll
@@ -138,6 +149,11 @@ forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, c
                 const float *p = base + (rowoff[q] + off_i);
                 acc[q] = fmaf(wlo, __ldg(p), acc[q]);
                 acc[q] = fmaf(whi, __ldg(p + 1), acc[q]);
+                if constexpr (MIRROR) {
+                    const float *pm = base + ((row_top - rowoff[q]) + off_i);
+                    accM[q] = fmaf(wlo, __ldg(pm), accM[q]);
+                    accM[q] = fmaf(whi, __ldg(pm + 1), accM[q]);
+                }
             }
             // Pass 2: a ray that crosses a z plane inside the slab (b < 1) moves its exit-row fractions
             // a - min(a,b) (row ja) and 1 - max(a,b) (row ja+dir) to the next z row, and continues there.
@@ -153,6 +169,11 @@ forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, c
                     const float c_lo = dneg ? c_r1 : c_r0, c_hi = dneg ? c_r0 : c_r1;
                     acc[q] = fmaf(c_lo, __ldg(p1) - __ldg(p), acc[q]);
                     acc[q] = fmaf(c_hi, __ldg(p1 + 1) - __ldg(p + 1), acc[q]);
+                    if constexpr (MIRROR) {
+                        const float *pm = base + ((row_top - rowoff[q]) + off_i), *pm1 = base + ((row_top - rowoff1) + off_i);
+                        accM[q] = fmaf(c_lo, __ldg(pm1) - __ldg(pm), accM[q]);
+                        accM[q] = fmaf(c_hi, __ldg(pm1 + 1) - __ldg(pm + 1), accM[q]);
+                    }
                     zbnd[q] += zs;
                     rowoff[q] = rowoff1;
                 }
@@ -165,13 +186,22 @@ forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, c
         const int v = v0 + q;
         if (v < d.nv) {
             const float len = chord_scale(r, __ldg(d.dz_mm + v));
-            const size_t o = ((size_t)a * d.nv + v) * d.nu + u;
-            float val = len * acc[q];
-            if (mode == 1) val = len * (val - __ldg(Y + o));
-            else if (mode == 2) val -= __ldg(Y + o);
-            out[o] = val;
+#pragma unroll
+            for (int m = 0; m < (MIRROR ? 2 : 1); ++m) {
+                const size_t o = ((size_t)a * d.nv + (m ? d.nv - 1 - v : v)) * d.nu + u;
+                float val = len * (m ? accM[MIRROR ? q : 0] : acc[q]);
+                if (mode == 1) val = len * (val - __ldg(Y + o));
+                else if (mode == 2) val -= __ldg(Y + o);
+                out[o] = val;
+            }
         }
     }
+}
+
+// the scan is its own mirror image about the central plane: even slice and detector-row counts, detector centred in v
+bool march_is_mirrored(const cbct_geometry *g)
+{
+    return g->use_mirror && g->nz % 2 == 0 && g->nv % 2 == 0 && g->off_v == 0.0;
 }
 
 cbct_status op_forward_padded(cbct_geometry *g, float *d_out, const float *d_Y, int mode, cudaStream_t st)
@@ -180,6 +210,9 @@ cbct_status op_forward_padded(cbct_geometry *g, float *d_out, const float *d_Y, 
 #ifndef CBCT_FW_V
 #define CBCT_FW_V 4
 #define CBCT_FW_WARPS 4
+#endif
+#ifndef CBCT_FW_VM
+#define CBCT_FW_VM 3
 #endif
     constexpr int V = CBCT_FW_V, WARPS = CBCT_FW_WARPS;
     if (g->fw_staged) {
@@ -190,10 +223,17 @@ cbct_status op_forward_padded(cbct_geometry *g, float *d_out, const float *d_Y, 
     ProfileScope ps(1, st);
     // every ray belongs to a tile of its class (geometry.cu), so every output element is written: 0 / -Y / -l Y for a
     // ray that misses the volume
+    const bool mirror = march_is_mirrored(g);
     for (int c = 0; c < 2; ++c) {
         if (g->n_tiles[c] == 0) continue;
-        dim3 grid(g->n_tiles[c], (g->nv + V * WARPS - 1) / (V * WARPS)), block(32, WARPS);
-        forward_kernel<V, WARPS><<<grid, block, 0, st>>>(g->dev, c, g->d_tiles[c], g->vol_pad[c], d_out, d_Y, mode);
+        if (mirror) {
+            constexpr int VM = CBCT_FW_VM;                    // ray pairs per thread
+            dim3 grid(g->n_tiles[c], (g->nv / 2 + VM * WARPS - 1) / (VM * WARPS)), block(32, WARPS);
+            forward_kernel<VM, WARPS, true><<<grid, block, 0, st>>>(g->dev, c, g->d_tiles[c], g->vol_pad[c], d_out, d_Y, mode);
+        } else {
+            dim3 grid(g->n_tiles[c], (g->nv + V * WARPS - 1) / (V * WARPS)), block(32, WARPS);
+            forward_kernel<V, WARPS, false><<<grid, block, 0, st>>>(g->dev, c, g->d_tiles[c], g->vol_pad[c], d_out, d_Y, mode);
+        }
         CBCT_LAUNCH_CHECK();
     }
     return CBCT_OK;
