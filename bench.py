@@ -156,6 +156,10 @@ def run_gpu(args):
     # replicas only: every rank runs its own copy of the same seeded scan; no data-path collective
     Y = np.ascontiguousarray(cfg.projections(), dtype=np.float32)
     G = cb.Geometry.from_synth(g)
+    if args.staged_projector:
+        G.set_projector_staging(True)
+    if args.plain_kernels:
+        G.set_mirror_symmetry(False)
     n_outer = [1] * LEVELS
     lv = level_dims(G, LEVELS)
     updates = 2.0 * sum(nvox * g.n_angles for nvox, _ in lv)
@@ -299,7 +303,9 @@ def run_gpu(args):
                                "step = 2-level FBS cascade, 1 outer iteration per level, 10 TV sweeps",
                    "levels": LEVELS, "n_tv_inner": N_INNER, "updates_per_step": updates,
                    "l2": "flushed between steps (256 MiB write); per-step working set ~0.9 GB > 126 MB L2",
-                   "parallelism": "replicas only (one independent reconstruction per GPU)" if world > 1 else "1 GPU"},
+                   "parallelism": "replicas only (one independent reconstruction per GPU)" if world > 1 else "1 GPU",
+                   "kernels": ("TMA-staged projector" if args.staged_projector else "cached march") +
+                              (", plain (unmirrored) march and gather" if args.plain_kernels else ", z-mirrored march and gather")},
         "clocks": clk.summary(),
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": 1e3 * t_e2e / K,
                 "h2d_bytes_per_step": int(h_Y.numel() * 4 + h_f.numel() * 4), "d2h_bytes_per_step": int(h_f.numel() * 4)},
@@ -508,6 +514,10 @@ def main():
     ap.add_argument("--cpu-angles", type=int, default=8)
     ap.add_argument("--shard-angles", action="store_true",
                     help="NEXT-4: shard the views of ONE reconstruction over the ranks (strong scaling) instead of replicas")
+    ap.add_argument("--staged-projector", action="store_true",
+                    help="measured variant: the TMA-staged projector (cbct_set_projector_staging) instead of the cached march")
+    ap.add_argument("--plain-kernels", action="store_true",
+                    help="measured variant: the plain march and gather (cbct_set_mirror_symmetry off) instead of the mirrored ones")
     ap.add_argument("--rank-probe", action="store_true",
                     help="every rank prints its RANK/LOCAL_RANK/WORLD_SIZE and exits (checks the launcher without a GPU)")
     args = ap.parse_args()
