@@ -158,8 +158,15 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
         for (int u = uA; u <= uB; ++u) {
             const RayXY r = load_ray(d, a, u);
             if (ray_cls(r.range) != cls) continue;
-            float a_, fl;
-            minor_split(ef, r, r.sm >= 0.f ? 1.f : 0.f, a_, fl);
+            // the projector's minor_split() with the minor coordinate Ya = mc + ef sm carried as two floats (exact product and
+            // sum, plus what the table's floats drop of mc and sm): the split a = (row boundary - Ya) / sm amplifies an error of
+            // Ya by 1 / |sm|, and fp32 leaves 1.5e-5 of a voxel in Ya at |ef| = 256
+            const float4 rlo = __ldg(d.rays_lo + (a * d.nu + u));
+            const float pm = __fmul_rn(ef, r.sm), pm_lo = fmaf(ef, r.sm, -pm);
+            const float Ya = __fadd_rn(r.mc, pm);
+            const float Ya_lo = fmaf(ef, rlo.y, __fadd_rn(__fadd_rn(two_sum_err(r.mc, pm, Ya), pm_lo), rlo.x));
+            const float fl = floorf(Ya);
+            const float a_ = __saturatef(__fsub_rn(__fsub_rn(fl + (r.sm >= 0.f ? 1.f : 0.f), Ya), Ya_lo) * r.inv_sm);
             const int ja = (int)fl + cg.joff;
             float l0, l1;
             if (ja == j) { l0 = 0.f; l1 = a_; }
@@ -175,7 +182,7 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
             // (__fmul_rn / __fadd_rn / __fsub_rn are never contracted into FMAs, which would break the error-free sums)
             const float p_hi = __fmul_rn(ef, r.dt), p_lo = fmaf(ef, r.dt, -p_hi);
             const float T = __fadd_rn(r.tc, p_hi);
-            const float T_lo = two_sum_err(r.tc, p_hi, T) + p_lo;
+            const float T_lo = (two_sum_err(r.tc, p_hi, T) + p_lo) + rlo.z;
             const float Tn = fmaf(ef + 1.f, r.dt, r.tc);
             const float rT = rcp_approx(T);
             const float cT = __fmul_rn(d.hzdv_hi, rT), cTn = d.hzdv_hi * rcp_approx(Tn);          // d v / d z at entry / exit (T > 0)
@@ -205,7 +212,10 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
             // l1 - b = (l1 - (T / dt) rho) + (T / dt) delta' / (v - cv): the correction costs nothing per plane.
             const float P_hi = __fmul_rn(zk0, cT), P_lo = fmaf(zk0, cT, -P_hi);
             const float xT0 = __fadd_rn(cv, P_hi), xTn0 = fmaf(zk0, cTn, cv);
-            const float x_lo = (two_sum_err(cv, P_hi, xT0) + P_lo) + d.cv_lo;
+            // reference row on a 2^-8 grid, so that vs - xTc is exact for every detector row vs (both multiples of 2^-8 below 2^15),
+            // and what it drops of cv + zk0 cT
+            const float xTc = rintf(xT0 * 256.f) * (1.f / 256.f);
+            const float x_lo = __fadd_rn((two_sum_err(cv, P_hi, xT0) + P_lo) + d.cv_lo, __fsub_rn(xT0, xTc));
             // MIRROR: prefix row nv and projection row nv-1 of this (a, u): the mirrored bound nv - vT and ray nv-1-vs are one
             // IMAD.WIDE with the negated pitch away
             const char *CuT = opaque(Cu + (long long)d.nv * pitchC), *RuT = opaque(Ru + (long long)(d.nv - 1) * pitchR);
@@ -240,9 +250,9 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
                     // crosses nothing: its 0 * inf is a NaN that the saturation turns into 0.
                     const int dlt = vTn - vT, vs = min(vT, vTn);
                     const float vsf = (float)vs, vf = vsf - cv;
-                    // delta = vs - (cv + (zk0 + q) cT): vs - xT0 is exact (both below 2^11 and a few rows apart), the FMA rounds a
-                    // number of a few rows at most, x_lo restores what xT0 dropped
-                    const float dl = __fsub_rn(fmaf(-(float)q, cT, __fsub_rn(vsf, xT0)), x_lo);
+                    // delta = vs - (cv + (zk0 + q) cT): vs - xTc is exact, the FMA rounds a number of a few rows at most, x_lo restores
+                    // what xTc dropped
+                    const float dl = __fsub_rn(fmaf(-(float)q, cT, __fsub_rn(vsf, xTc)), x_lo);
                     const float fr = fminf(__saturatef(fmaf(TD, dl * rcp_approx(vf), l1c)), w);
                     // signed: positive = the ray rises across the plane (dt zeta(v) > 0), so the fraction moves from the row below
                     // the plane to the row above it
@@ -263,7 +273,7 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
                     }
                     if constexpr (MULTI) {
                         for (int v = vs + 1; v < vs + abs(dlt); ++v) {   // further rays crossing this plane (fine detector rows)
-                            const float dl2 = __fsub_rn(fmaf(-(float)q, cT, __fsub_rn((float)v, xT0)), x_lo);
+                            const float dl2 = __fsub_rn(fmaf(-(float)q, cT, __fsub_rn((float)v, xTc)), x_lo);
                             const float fr2 = fminf(__saturatef(fmaf(TD, dl2 * rcp_approx((float)v - cv), l1c)), w);
                             const float f2 = __int_as_float(__float_as_int(fr2) ^ sgn);
                             up = fmaf(f2, __ldg(reinterpret_cast<const float *>(row_ptr(Ru, v, pitchR))), up);

@@ -54,6 +54,7 @@ struct DevGeom {
     float hzdv_hi, hzdv_lo;     // hz / dv as an unevaluated sum of two floats (the gather places z planes on the detector with it)
     ClassGrid cls[2];
     const RayXY *rays;          // [na][nu]
+    const float4 *rays_lo;      // [na][nu]  what the floats mc, sm, tc of RayXY drop of their fp64 values (x, y, z); read by the gather
     const float *zeta;          // [nv]  Dz(v)/hz
     const float *inv_zeta;      // [nv]  hz/Dz(v) (+-1e30 if Dz == 0)
     const float *dz_mm;         // [nv]  Dz(v) in mm
@@ -71,6 +72,7 @@ struct cbct_geometry {
     DevGeom dev{};
     // device tables
     RayXY *d_rays = nullptr;
+    float4 *d_rays_lo = nullptr;
     float *d_zeta = nullptr, *d_inv_zeta = nullptr, *d_dz = nullptr;
     float2 *d_cs = nullptr;
     int2 *d_tiles[2] = {nullptr, nullptr};   // forward work list per class: (angle, u0)

@@ -41,7 +41,7 @@ static void free_handle(cbct_geometry *g)
 {
     if (!g) return;
     free_handle(g->coarse);
-    void *ptrs[] = {g->d_rays, g->d_zeta, g->d_inv_zeta, g->d_dz, g->d_cs, g->d_tiles[0], g->d_tiles[1],
+    void *ptrs[] = {g->d_rays, g->d_rays_lo, g->d_zeta, g->d_inv_zeta, g->d_dz, g->d_cs, g->d_tiles[0], g->d_tiles[1],
                     g->d_angle_has[0], g->d_angle_has[1], g->vol_pad[0], g->vol_pad[1], g->proj_tmp, g->proj_prefix,
                     g->G_cls[0], g->G_cls[1], g->vol_a, g->vol_b, g->vol_c, g->vol_f, g->Y_level, g->vc_tau, g->vc_f0, g->vc_d, g->vc_e, g->fdk_q, g->fdk_hk,
                     g->red_partial, g->red_out, g->host_stage_vol, g->host_stage_proj, g->host_stage_vol2};
@@ -113,6 +113,7 @@ static cbct_status build_tables(cbct_geometry *g)
     }
 
     std::vector<RayXY> rays((size_t)na * nu);
+    std::vector<float4> rays_lo((size_t)na * nu);
     std::vector<float2> cs(na);
     std::vector<float> zeta(nv), inv_zeta(nv), dz(nv);
     double max_abs_zeta = 0.0;
@@ -171,6 +172,8 @@ static cbct_status build_tables(cbct_geometry *g)
             if (ihi < ilo) ihi = ilo;
             r.range = ilo | (ihi << 15) | (c << 30);
             rays[(size_t)a * nu + u] = r;
+            rays_lo[(size_t)a * nu + u] = make_float4((float)((mcu - cg.joff) - (double)r.mc), (float)(sm - (double)r.sm),
+                                                      (float)(tc - (double)r.tc), 0.f);
             if (ihi > ilo) {
                 g->h_angle_has[c][a] = 1;
                 max_abs_dt = std::fmax(max_abs_dt, std::fabs(dt));
@@ -194,6 +197,7 @@ static cbct_status build_tables(cbct_geometry *g)
         return CBCT_ERR_SHAPE;
     }
     CBCT_TRY(upload(g, &g->d_rays, rays));
+    CBCT_TRY(upload(g, &g->d_rays_lo, rays_lo));
     CBCT_TRY(upload(g, &g->d_cs, cs));
     CBCT_TRY(upload(g, &g->d_zeta, zeta));
     CBCT_TRY(upload(g, &g->d_inv_zeta, inv_zeta));
@@ -203,7 +207,7 @@ static cbct_status build_tables(cbct_geometry *g)
         CBCT_TRY(upload(g, &g->d_tiles[c], tiles[c]));
         CBCT_TRY(upload(g, &g->d_angle_has[c], g->h_angle_has[c]));
     }
-    d.rays = g->d_rays; d.cs = g->d_cs; d.zeta = g->d_zeta; d.inv_zeta = g->d_inv_zeta; d.dz_mm = g->d_dz;
+    d.rays = g->d_rays; d.rays_lo = g->d_rays_lo; d.cs = g->d_cs; d.zeta = g->d_zeta; d.inv_zeta = g->d_inv_zeta; d.dz_mm = g->d_dz;
     // the table uploads are cudaMemcpy's from pageable memory on the legacy default stream: wait for them here, so that the
     // first kernel may run on any (also a non-blocking) stream
     CBCT_CUDA(cudaStreamSynchronize(nullptr));
