@@ -208,25 +208,55 @@ cbct_status op_fbs_level(cbct_geometry *g, const float *d_Y, float *f, int n_out
     CBCT_TRY(ensure(g, &g->vol_a, g->n_vox()));
     const float beta = mu / step;
     const float c = (float)(2.0 * (double)step * (double)g->n_vox() / ((double)g->na * g->nu * g->nv));
-    for (int it = 0; it < n_outer; ++it) {
-        if (rel_tol > 0.f) CBCT_CUDA(cudaMemcpyAsync(g->vol_c, f, g->n_vox() * sizeof(float), cudaMemcpyDeviceToDevice, st));
-        CBCT_TRY(op_pad_copies(g, f, st));
+    // one outer iteration (steps 1-3 of A1) on stream s: the same launches with the same arguments every iteration
+    auto iteration = [&](cudaStream_t s) -> cbct_status {
+        CBCT_TRY(op_pad_copies(g, f, s));
         if (g->bp_mode == CBCT_BACKPROJECTOR_EQ2) {
             // the paper's step 1 (P:87 with eq. 2): dE2/df = (2/(N_theta A)) B r, so gv = f - c (dV/(du dv)) B r
             const float c2 = (float)((double)c * (g->hx * g->hy * g->hz) / (g->du * g->dv));
-            CBCT_TRY(op_forward_padded(g, g->proj_tmp, d_Y, 2, st));      // P f - Y              a1+a2
-            CBCT_TRY(op_backproject_eq2(g, g->proj_tmp, f, c2, n_inner == 0 && !tau, g->vol_a, st));   // a3 (eq. 2) + a4 (+ a6)
-            if (tau) CBCT_TRY(op_axpy_clamp(g, g->vol_a, tau, -1.f / beta, n_inner == 0, g->vol_a, st));
-            if (n_inner == 0) CBCT_CUDA(cudaMemcpyAsync(f, g->vol_a, g->n_vox() * sizeof(float), cudaMemcpyDeviceToDevice, st));
-            else CBCT_TRY(tv_inner(g, g->vol_a, g->vol_a, f, beta, eps, omega, n_inner, 1, st));
+            CBCT_TRY(op_forward_padded(g, g->proj_tmp, d_Y, 2, s));      // P f - Y              a1+a2
+            CBCT_TRY(op_backproject_eq2(g, g->proj_tmp, f, c2, n_inner == 0 && !tau, g->vol_a, s));   // a3 (eq. 2) + a4 (+ a6)
+            if (tau) CBCT_TRY(op_axpy_clamp(g, g->vol_a, tau, -1.f / beta, n_inner == 0, g->vol_a, s));
+            if (n_inner == 0) CBCT_CUDA(cudaMemcpyAsync(f, g->vol_a, g->n_vox() * sizeof(float), cudaMemcpyDeviceToDevice, s));
+            else CBCT_TRY(tv_inner(g, g->vol_a, g->vol_a, f, beta, eps, omega, n_inner, 1, s));
         } else {
-            CBCT_TRY(op_forward_padded(g, g->proj_tmp, d_Y, 1, st));          // l (P f - Y)          a1+a2
-            CBCT_TRY(op_backproject_prefix(g, g->proj_tmp, 0, nullptr, st));
-            CBCT_TRY(op_backproject_gather(g, g->proj_tmp, st));              // P^T (P f - Y)        a3
-            CBCT_TRY(op_combine(g, f, c, n_inner == 0 && !tau, g->vol_a, st));    // gv = f - c G (a4), clamped (a6) if nothing follows
-            if (tau) CBCT_TRY(op_axpy_clamp(g, g->vol_a, tau, -1.f / beta, n_inner == 0, g->vol_a, st));   // + tau / beta
-            if (n_inner == 0) CBCT_CUDA(cudaMemcpyAsync(f, g->vol_a, g->n_vox() * sizeof(float), cudaMemcpyDeviceToDevice, st));
-            else CBCT_TRY(tv_inner(g, g->vol_a, g->vol_a, f, beta, eps, omega, n_inner, 1, st));   // u0 = gv (Q7); a5 + a6
+            CBCT_TRY(op_forward_padded(g, g->proj_tmp, d_Y, 1, s));          // l (P f - Y)          a1+a2
+            CBCT_TRY(op_backproject_prefix(g, g->proj_tmp, 0, nullptr, s));
+            CBCT_TRY(op_backproject_gather(g, g->proj_tmp, s));              // P^T (P f - Y)        a3
+            CBCT_TRY(op_combine(g, f, c, n_inner == 0 && !tau, g->vol_a, s));    // gv = f - c G (a4), clamped (a6) if nothing follows
+            if (tau) CBCT_TRY(op_axpy_clamp(g, g->vol_a, tau, -1.f / beta, n_inner == 0, g->vol_a, s));   // + tau / beta
+            if (n_inner == 0) CBCT_CUDA(cudaMemcpyAsync(f, g->vol_a, g->n_vox() * sizeof(float), cudaMemcpyDeviceToDevice, s));
+            else CBCT_TRY(tv_inner(g, g->vol_a, g->vol_a, f, beta, eps, omega, n_inner, 1, s));   // u0 = gv (Q7); a5 + a6
+        }
+        return CBCT_OK;
+    };
+    // Small volumes are launch-bound (c1: a dozen kernels of 5-10 us per iteration): after one eager iteration (which makes
+    // every allocation) the iteration is captured once into a CUDA graph on an internal stream and replayed on the caller's.
+    // Any failure to capture falls back to eager launches.
+    cudaGraphExec_t gexec = nullptr;
+    const bool want_graph = !trace && rel_tol == 0.f && !cbct_profile_is_on() && n_outer >= 6 && g->n_vox() <= ((size_t)1 << 20);
+    for (int it = 0; it < n_outer; ++it) {
+        if (rel_tol > 0.f) CBCT_CUDA(cudaMemcpyAsync(g->vol_c, f, g->n_vox() * sizeof(float), cudaMemcpyDeviceToDevice, st));
+        if (want_graph && it == 1 && !gexec) {
+            if (!g->graph_stream && cudaStreamCreateWithFlags(&g->graph_stream, cudaStreamNonBlocking) != cudaSuccess) g->graph_stream = nullptr;
+            cudaGraph_t graph = nullptr;
+            if (g->graph_stream && cudaStreamBeginCapture(g->graph_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+                const unsigned long long n0 = g_cbct_launches.load();
+                const cbct_status cs = iteration(g->graph_stream);           // recorded, not run
+                g_cbct_launches.store(n0);
+                const cudaError_t ce = cudaStreamEndCapture(g->graph_stream, &graph);
+                if (cs != CBCT_OK || ce != cudaSuccess || !graph || cudaGraphInstantiate(&gexec, graph, 0) != cudaSuccess) gexec = nullptr;
+                if (graph) cudaGraphDestroy(graph);
+            }
+            (void)cudaGetLastError();                            // a failed capture leaves no sticky error behind
+        }
+        if (gexec && it >= 1) {
+            CBCT_CUDA(cudaGraphLaunch(gexec, st));
+            g_cbct_launches += g->launches_per_iteration;
+        } else {
+            const unsigned long long n0 = g_cbct_launches.load();
+            CBCT_TRY(iteration(st));
+            g->launches_per_iteration = g_cbct_launches.load() - n0;
         }
         if (trace) {
             double e3[3];
@@ -242,6 +272,7 @@ cbct_status op_fbs_level(cbct_geometry *g, const float *d_Y, float *f, int n_out
             if (std::sqrt(g->h_red[0]) <= (double)rel_tol * std::sqrt(g->h_red[1])) break;
         }
     }
+    if (gexec) cudaGraphExecDestroy(gexec);
     return CBCT_OK;
 }
 

@@ -103,6 +103,9 @@ struct cbct_geometry {
     int fw_bj[2] = {0, 0}, fw_bk[2] = {0, 0};  // brick spans per class (0 = not computed yet)
     int bin_detector = 1;                     // coarse levels bin the detector 2x2 (O6) or keep it at full resolution (Q20)
 
+    cudaStream_t graph_stream = nullptr;      // internal stream the outer iteration of a small volume is captured on (api.cu)
+    unsigned long long launches_per_iteration = 0;   // kernels one outer iteration launches (counted on an eager one)
+
     // multigrid
     cbct_geometry *coarse = nullptr;
     int coarsen_flags[4] = {0, 0, 0, 0};
@@ -140,6 +143,7 @@ extern std::atomic<unsigned long long> g_cbct_launches;
     } while (0)
 
 // ---- per-kernel-class event timing (profile.cu) ---------------------------------------------
+bool cbct_profile_is_on();
 struct ProfileScope {
     ProfileScope(int tag, cudaStream_t st);
     ~ProfileScope();

@@ -48,6 +48,7 @@ static void free_handle(cbct_geometry *g)
     for (void *p : ptrs)
         if (p) cudaFree(p);
     if (g->h_red) cudaFreeHost(g->h_red);
+    if (g->graph_stream) cudaStreamDestroy(g->graph_stream);
     delete g;
 }
 

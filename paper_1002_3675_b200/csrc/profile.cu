@@ -19,6 +19,8 @@ cudaEvent_t get_event()
 }
 }  // namespace
 
+bool cbct_profile_is_on() { return g_on; }
+
 ProfileScope::ProfileScope(int tag, cudaStream_t st) : tag_(tag), st_(st), a_(nullptr)
 {
     if (!g_on) return;
