@@ -54,22 +54,57 @@ __device__ __forceinline__ float two_sum_err(float a, float b, float s)
     return __fadd_rn(__fsub_rn(a, __fsub_rn(s, bb)), __fsub_rn(b, bb));
 }
 
+#ifndef CBCT_BP_FIXED
+#define CBCT_BP_FIXED 0
+#endif
+// Prefix sums along v in one of two forms.  kFixed = false: (sum, two-sum compensation) float pairs.  kFixed = true: 32-bit
+// fixed point with wrap-around: every column (a, u) is scaled by a power of two s(a,u) such that any run of at most
+// `run_max` detector rows sums to less than 2^30 in magnitude, rounded to integers and summed modulo 2^32, so the difference
+// of two prefix values is the EXACT sum of the rounded run whatever the prefix has grown to; 1/s(a,u) sits in a float table
+// behind the prefix values.  Half the bytes per lookup and one integer subtraction per run.
+constexpr bool kFixed = CBCT_BP_FIXED != 0;
+using PrefixT = std::conditional_t<kFixed, int, float2>;
+__device__ __forceinline__ float run_sum(const float2 hi, const float2 lo) { return (hi.x - lo.x) + (hi.y - lo.y); }
+__device__ __forceinline__ float run_sum(const int hi, const int lo) { return (float)(hi - lo); }
+__device__ __forceinline__ void put_prefix(float2 *p, float s, float e, unsigned) { *p = make_float2(s, e); }
+__device__ __forceinline__ void put_prefix(int *p, float, float, unsigned si) { *p = (int)si; }
+
 // C[a][v][u] = sum_{v' < v} y[a][v'][u] for v = 0..nv as (sum, compensation) pairs: the rounding
 // error of every addition is carried in the second float (two-sum), so C(v2) - C(v1) evaluated as
 // (s2 - s1) + (c2 - c1) has the accuracy of summing the run directly.
 // scale != 0: y = l(u,v) * in (and the scaled projections are also written to rs_out).
 __global__ void __launch_bounds__(128) prefix_kernel(const DevGeom d, const float *__restrict__ in, const int scale,
-                                                     float *__restrict__ rs_out, float2 *__restrict__ C)
+                                                     float *__restrict__ rs_out, PrefixT *__restrict__ C, float *__restrict__ inv_s,
+                                                     const float run_max)
 {
     const int u = blockIdx.x * blockDim.x + threadIdx.x, a = blockIdx.y;
     if (u >= d.nu) return;
     RayXY r = load_ray(d, a, u);
     const float *p = in + (size_t)a * d.nv * d.nu + u;
     float *po = rs_out ? rs_out + (size_t)a * d.nv * d.nu + u : nullptr;
-    float2 *c = C + (size_t)a * (d.nv + 1) * d.nu + u;
-    float s = 0.f, e = 0.f;
-    *c = make_float2(0.f, 0.f);
+    PrefixT *c = C + (size_t)a * (d.nv + 1) * d.nu + u;
     constexpr int PF = 8;
+    float sc = 1.f;                                        // kFixed: the column's power-of-two scale
+    if constexpr (kFixed) {
+        float m = 0.f;
+        for (int v0 = 0; v0 < d.nv; v0 += PF) {
+            float y[PF];
+#pragma unroll
+            for (int q = 0; q < PF; ++q) y[q] = (v0 + q < d.nv) ? __ldg(p + (size_t)(v0 + q) * d.nu) : 0.f;
+#pragma unroll
+            for (int q = 0; q < PF; ++q) {
+                if (v0 + q >= d.nv) break;
+                m = fmaxf(m, fabsf(scale ? y[q] * chord_scale(r, __ldg(d.dz_mm + v0 + q)) : y[q]));
+            }
+        }
+        int e = 0;
+        frexpf(m * run_max, &e);                           // m run_max = f 2^e, f in [0.5, 1): f 2^30 < 2^30
+        sc = (m > 0.f && m < 3e38f) ? ldexpf(1.f, max(min(30 - e, 120), -120)) : 1.f;
+        inv_s[(size_t)a * d.nu + u] = 1.f / sc;
+    }
+    float s = 0.f, e = 0.f;
+    unsigned si = 0u;
+    put_prefix(c, 0.f, 0.f, 0u);
     for (int v0 = 0; v0 < d.nv; v0 += PF) {
         float y[PF];
 #pragma unroll
@@ -82,11 +117,15 @@ __global__ void __launch_bounds__(128) prefix_kernel(const DevGeom d, const floa
                 yy *= chord_scale(r, __ldg(d.dz_mm + v0 + q));
                 if (po) po[(size_t)(v0 + q) * d.nu] = yy;
             }
-            const float t = s + yy;
-            const float bp = t - s;
-            e += (s - (t - bp)) + (yy - bp);
-            s = t;
-            c[(size_t)(v0 + q + 1) * d.nu] = make_float2(s, e);
+            if constexpr (kFixed) {
+                si += (unsigned)__float2int_rn(yy * sc);
+            } else {
+                const float t = s + yy;
+                const float bp = t - s;
+                e += (s - (t - bp)) + (yy - bp);
+                s = t;
+            }
+            put_prefix(c + (size_t)(v0 + q + 1) * d.nu, s, e, si);
         }
     }
 }
@@ -107,7 +146,8 @@ __global__ void __launch_bounds__(128) prefix_kernel(const DevGeom d, const floa
 template <int KC, int BI, bool MIRROR>
 __global__ void __launch_bounds__(32 * BI, MIRROR ? CBCT_BP_MINB_M : CBCT_BP_MINB)
 backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restrict__ angle_has,
-                   const float *__restrict__ rs, const float2 *__restrict__ C, float *__restrict__ G, const int parts)
+                   const float *__restrict__ rs, const PrefixT *__restrict__ C, const float *__restrict__ inv_s, float *__restrict__ G,
+                   const int parts)
 {
     const ClassGrid cg = d.cls[cls];
     const int j = blockIdx.x * 32 + threadIdx.x;      // minor index
@@ -136,7 +176,7 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
     const float ef = (float)(i - cg.ioff);
     const float cu = d.cu, cv = d.cv;                  // detector index of the central ray (shifted panels: not the middle)
     const float sdd_du = d.sdd / d.du;
-    const int npitchC = opaque(-d.nu * (int)sizeof(float2)), npitchR = opaque(-d.nu * (int)sizeof(float));   // MIRROR: rows counted down
+    const int npitchC = opaque(-d.nu * (int)sizeof(PrefixT)), npitchR = opaque(-d.nu * (int)sizeof(float));   // MIRROR: rows counted down
     const float inv_hzdv = rcp_approx(d.hzdv_hi);
     const float zk0 = (float)(k0 - d.koff) - d.zfrac;  // plane k0 in the units of z_entry(), minus zfrac (MIRROR: >= 0, an integer)
 
@@ -191,8 +231,9 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
             // 32-bit element offsets of (a, v = 0, u) in the prefix sums and in the projections (checked at geometry creation)
             // byte offsets: one IMAD.WIDE (row * pitch + base) forms the address of a row's element
             const char *Cu = reinterpret_cast<const char *>(C + (a * (d.nv + 1) * d.nu + u));
+            const float wr = kFixed ? w * __ldg(inv_s + (a * d.nu + u)) : w;          // weight of a run sum (fixed point: unscaled)
             const char *Ru = reinterpret_cast<const char *>(rs + (a * d.nv * d.nu + u));
-            const int pitchC = d.nu * (int)sizeof(float2), pitchR = d.nu * (int)sizeof(float);
+            const int pitchC = d.nu * (int)sizeof(PrefixT), pitchR = d.nu * (int)sizeof(float);
             // b = lambda at which ray v meets plane zk: (T + b dt) (v - cv) dv / hz = zk.  With delta = (v - cv) - zk cT, the
             // distance of the ray from where the plane meets the detector at the slab's entry, b = -(T / dt) delta / (v - cv).
             const float TD = T * r.inv_dt;
@@ -222,7 +263,7 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
             const int up_sign = __float_as_int(r.dt) & 0x80000000;                     // MIRROR: rising iff dt > 0
             auto planes = [&](auto multi_tag, auto clamp_tag) {
                 constexpr bool MULTI = decltype(multi_tag)::value, CLAMP = decltype(clamp_tag)::value;
-                float2 c1 = make_float2(0.f, 0.f), c1L = make_float2(0.f, 0.f);
+                PrefixT c1{}, c1L{};
 #pragma unroll
                 for (int q = 0; q <= KC; ++q) {
                     // first ray at or above plane k0+q at the slab's entry / exit plane
@@ -242,7 +283,7 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
                         vT = min(max(vT, 0), d.nv);
                         vTn = min(max(vTn, 0), d.nv);
                     }
-                    const float2 c2 = __ldg(reinterpret_cast<const float2 *>(row_ptr(Cu, vT, pitchC)));
+                    const PrefixT c2 = __ldg(reinterpret_cast<const PrefixT *>(row_ptr(Cu, vT, pitchC)));
                     // rays crossing plane k0+q inside the slab: v in [min(vT,vTn), max(vT,vTn)) (y = 0 stands in if there is none).
                     // The part of such a ray's chord in this minor row that lies beyond the plane is
                     //   max(0, l1 - max(l0, sat(b))) = min(sat(l1 - b), l1 - l0)       (0 <= l0 <= l1 <= 1)
@@ -263,10 +304,10 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
                     float up = fs * yq;                // moved up across the plane (negative: moved down)
                     // the mirror image: plane -zk, bounds nv - vT (plane 0 is its own image: the same bound, so that a ray lying
                     // in it belongs to the row above it on both sides), crossing ray nv-1-vs, rising <-> falling
-                    [[maybe_unused]] float2 c2L;
+                    [[maybe_unused]] PrefixT c2L;
                     [[maybe_unused]] float dn = 0.f;                    // moved DOWN across the mirrored plane
                     if constexpr (MIRROR) {
-                        c2L = (q == 0 && zk0 == 0.f) ? c2 : __ldg(reinterpret_cast<const float2 *>(row_ptr(CuT, vT, npitchC)));
+                        c2L = (q == 0 && zk0 == 0.f) ? c2 : __ldg(reinterpret_cast<const PrefixT *>(row_ptr(CuT, vT, npitchC)));
                         float yL = 0.f;
                         if (dlt != 0) yL = __ldg(reinterpret_cast<const float *>(row_ptr(RuT, vs, npitchR)));
                         dn = fs * yL;
@@ -281,11 +322,9 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
                         }
                     }
                     if (q > 0) {
-                        const float ysum = (c2.x - c1.x) + (c2.y - c1.y);
-                        acc[q > 0 ? q - 1 : 0] = fmaf(w, ysum, acc[q > 0 ? q - 1 : 0]) - up;
+                        acc[q > 0 ? q - 1 : 0] = fmaf(wr, run_sum(c2, c1), acc[q > 0 ? q - 1 : 0]) - up;
                         if constexpr (MIRROR) {
-                            const float ysumL = (c1L.x - c2L.x) + (c1L.y - c2L.y);
-                            accL[q > 0 ? q - 1 : 0] = fmaf(w, ysumL, accL[q > 0 ? q - 1 : 0]) - dn;
+                            accL[q > 0 ? q - 1 : 0] = fmaf(wr, run_sum(c1L, c2L), accL[q > 0 ? q - 1 : 0]) - dn;
                         }
                     }
                     if (q < KC) {
@@ -317,7 +356,10 @@ cbct_status op_backproject_prefix(cbct_geometry *g, const float *d_in, int scale
     CBCT_TRY(ensure(g, &g->proj_prefix, (size_t)g->na * (g->nv + 1) * g->nu));
     ProfileScope ps(2, st);
     dim3 grid((g->nu + 127) / 128, g->na);
-    prefix_kernel<<<grid, 128, 0, st>>>(g->dev, d_in, scale, d_rs_out, g->proj_prefix);
+    // kFixed: the column scales 1/s(a,u) sit behind the (half-size) integer prefix values in the same buffer
+    PrefixT *Cp = reinterpret_cast<PrefixT *>(g->proj_prefix);
+    float *inv_s = kFixed ? reinterpret_cast<float *>(Cp + (size_t)g->na * (g->nv + 1) * g->nu) : nullptr;
+    prefix_kernel<<<grid, 128, 0, st>>>(g->dev, d_in, scale, d_rs_out, Cp, inv_s, g->bp_run_max);
     CBCT_LAUNCH_CHECK();
     return CBCT_OK;
 }
@@ -346,7 +388,9 @@ static cbct_status launch_gather(cbct_geometry *g, const float *d_scaled, cudaSt
         }
         const ClassGrid &cg = g->dev.cls[c];
         dim3 grid((cg.nmin + 31) / 32, (cg.nmaj + BI - 1) / BI, kchunks * g->bp_parts), block(32, BI);
-        backproject_kernel<KC, BI, MIRROR><<<grid, block, 0, st>>>(g->dev, c, g->d_angle_has[c], d_scaled, g->proj_prefix, g->G_cls[c], g->bp_parts);
+        const PrefixT *Cp = reinterpret_cast<const PrefixT *>(g->proj_prefix);
+        const float *inv_s = kFixed ? reinterpret_cast<const float *>(Cp + (size_t)g->na * (g->nv + 1) * g->nu) : nullptr;
+        backproject_kernel<KC, BI, MIRROR><<<grid, block, 0, st>>>(g->dev, c, g->d_angle_has[c], d_scaled, Cp, inv_s, g->G_cls[c], g->bp_parts);
         CBCT_LAUNCH_CHECK();
     }
     return CBCT_OK;
@@ -384,36 +428,49 @@ __global__ void __launch_bounds__(256) combine_kernel(const float *__restrict__ 
     const int k = blockIdx.z;
     const int i0 = blockIdx.x * 32, j0 = blockIdx.y * 32;
     const size_t plane = (size_t)k * nx * ny;
-    if (G0) {
-        // G0 is [k][x][y]: read rows of constant x
-        for (int r = threadIdx.y; r < 32; r += 8) {
-            int i = i0 + r, j = j0 + threadIdx.x;
-            float v = 0.f;
-            if (i < nx && j < ny) {
-                v = __ldg(G0 + plane + (size_t)i * ny + j);
-                if constexpr (PARTS)
-                    for (int p = 1; p < parts; ++p) v += __ldg(G0 + p * nvox + plane + (size_t)i * ny + j);
-            }
-            tile[r][threadIdx.x] = v;
+    // all of a thread's loads (4 of G0 for the transpose, 4 of G1, 4 of f) are requested before the first use: the kernel is
+    // latency-bound, so what counts is the bytes in flight
+    float g1[4], fv[4], g0[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const int r = threadIdx.y + 8 * q;
+        const int j = j0 + r, i = i0 + threadIdx.x;
+        const bool in = j < ny && i < nx;
+        const size_t o = plane + (size_t)j * nx + i;
+        g1[q] = 0.f;
+        if (G1 && in) {
+            g1[q] = __ldg(G1 + o);
+            if constexpr (PARTS)
+                for (int p = 1; p < parts; ++p) g1[q] += __ldg(G1 + p * nvox + o);
         }
+        fv[q] = (f && in) ? __ldg(f + o) : 0.f;
+        g0[q] = 0.f;
+        if (G0) {                                  // G0 is [k][x][y]: read rows of constant x
+            const int ii = i0 + r, jj = j0 + threadIdx.x;
+            if (ii < nx && jj < ny) {
+                g0[q] = __ldg(G0 + plane + (size_t)ii * ny + jj);
+                if constexpr (PARTS)
+                    for (int p = 1; p < parts; ++p) g0[q] += __ldg(G0 + p * nvox + plane + (size_t)ii * ny + jj);
+            }
+        }
+    }
+    if (G0) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) tile[threadIdx.y + 8 * q][threadIdx.x] = g0[q];
         __syncthreads();
     }
-    for (int r = threadIdx.y; r < 32; r += 8) {
-        int j = j0 + r, i = i0 + threadIdx.x;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const int r = threadIdx.y + 8 * q;
+        const int j = j0 + r, i = i0 + threadIdx.x;
         if (j < ny && i < nx) {
-            const size_t o = plane + (size_t)j * nx + i;
-            float gsum = G0 ? tile[threadIdx.x][r] : 0.f;
-            if (G1) {
-                gsum += __ldg(G1 + o);
-                if constexpr (PARTS)
-                    for (int p = 1; p < parts; ++p) gsum += __ldg(G1 + p * nvox + o);
-            }
+            const float gsum = (G0 ? tile[threadIdx.x][r] : 0.f) + g1[q];
             float val = gsum;
             if (f) {
-                val = fmaf(-c, gsum, __ldg(f + o));
+                val = fmaf(-c, gsum, fv[q]);
                 if (clamp) val = fmaxf(val, 0.f);
             }
-            out[o] = val;
+            out[plane + (size_t)j * nx + i] = val;
         }
     }
 }

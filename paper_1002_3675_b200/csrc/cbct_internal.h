@@ -80,6 +80,7 @@ struct cbct_geometry {
     unsigned char *d_angle_has[2] = {nullptr, nullptr};   // [na] does this angle have rays of the class
     std::vector<unsigned char> h_angle_has[2];
     float max_abs_sz = 0.f;
+    float bp_run_max = 2.f;                   // upper bound of the detector rows one voxel row's run can hold (fixed-point prefix sums)
 
     // lazily allocated scratch (device)
     float *vol_pad[2] = {nullptr, nullptr};   // padded [nz+2K][nmaj][row_stride] copies (class 0 transposed)

@@ -129,7 +129,7 @@ static cbct_status build_tables(cbct_geometry *g)
         max_abs_zeta = std::fmax(max_abs_zeta, std::fabs(Dz / g->hz));
     }
     std::vector<int2> tiles[2];
-    double max_abs_dt = 0.0;
+    double max_abs_dt = 0.0, t_min = 1.0;
     for (int c = 0; c < 2; ++c) g->h_angle_has[c].assign(na, 0);
     for (int a = 0; a < na; ++a) {
         const double th = g->angles[a], co = std::cos(th), si = std::sin(th);
@@ -178,6 +178,7 @@ static cbct_status build_tables(cbct_geometry *g)
             if (ihi > ilo) {
                 g->h_angle_has[c][a] = 1;
                 max_abs_dt = std::fmax(max_abs_dt, std::fabs(dt));
+                t_min = std::fmin(t_min, std::fmin(tc + (ilo - cg.ioff) * dt, tc + (ihi - cg.ioff) * dt));
             }
         }
         for (int c = 0; c < 2; ++c)
@@ -192,6 +193,7 @@ static cbct_status build_tables(cbct_geometry *g)
             }
     }
     g->max_abs_sz = (float)(max_abs_dt * max_abs_zeta);
+    g->bp_run_max = (float)(std::ceil((g->hz / g->dv) / std::fmax(t_min, 1e-3)) + 2.0);
     if (g->max_abs_sz > 0.999f) {
         cbct_set_error("geometry unsupported: a ray climbs %.3f voxels in z per major-axis voxel (limit 0.999)",
                        g->max_abs_sz);
