@@ -20,7 +20,9 @@
  *     synchronising it.
  *   - A handle owns per-angle ray tables and lazily allocated scratch (grown on first use, freed
  *     by cbct_geometry_destroy).  A handle must not be used from two host threads or two streams
- *     at the same time.
+ *     at the same time.  One CUDA device per process (the intended deployment is one process per GPU): kernel
+ *     attributes and occupancy figures are cached per process, the launch counter and the optional per-kernel timing
+ *     (cbct_profile_*) are process-wide.
  *   - Errors: every call returns a cbct_status; nothing throws or aborts across the ABI.  On
  *     failure outputs are unspecified and cbct_last_error() describes the failure (thread-local).
  *   - There is no CPU fallback: with no CUDA device every compute call returns CBCT_ERR_CUDA.
@@ -342,6 +344,16 @@ unsigned long long cbct_launch_count(void);
 
 /* Bytes of device memory currently held by the handle (tables + scratch, all levels). */
 unsigned long long cbct_device_bytes(const cbct_geometry *g);
+
+/*
+ * Debugging aid standing in for a memory checker: after cbct_set_guard_mode(1) every device buffer that a handle allocates
+ * (tables at creation, scratch on first use) is placed between two 4096-byte regions filled with a pattern (slower: every
+ * allocation synchronises the device).  cbct_check_guards synchronises the device and writes to *h_bad_bytes the number of
+ * pattern bytes around the buffers of this handle and of its coarse levels that no longer hold the pattern: 0 unless a kernel
+ * wrote outside a library-owned buffer.  Process-wide switch; affects allocations made after the call.
+ */
+cbct_status cbct_set_guard_mode(int on);
+cbct_status cbct_check_guards(const cbct_geometry *g, unsigned long long *h_bad_bytes);
 
 /* Description of the last failure on this host thread ("" if none).  Static storage. */
 const char *cbct_last_error(void);

@@ -9,7 +9,7 @@ missing, and every compute call fails if there is no CUDA device.
 from .binding import (  # noqa: F401
     CbctError, Geometry, load, lib_path, launch_count,
     forward, backproject, backproject_eq2, set_backprojector, BACKPROJECTOR_EXACT, BACKPROJECTOR_EQ2, tv_prox, fbs_reconstruct, fbs_reconstruct_until, data_gradient, prox_step, energy, prolong, restrict, bin2x2,
-    profile_enable, profile_read, PROFILE_TAGS,
+    profile_enable, profile_read, PROFILE_TAGS, set_guard_mode,
     forward_host, backproject_host, tv_prox_host, fbs_reconstruct_host,
     fbs_vcycle, fdk_reconstruct, fbs_reconstruct_sharded, CascadeOps, ALLREDUCE_FN,
 )

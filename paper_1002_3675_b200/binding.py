@@ -15,7 +15,7 @@ STATUS = {0: "CBCT_OK", 1: "CBCT_ERR_INVALID_ARG", 2: "CBCT_ERR_SHAPE", 3: "CBCT
 # every symbol include/cbct.h declares (tests check that the library exports each of them)
 SYMBOLS = (
     "cbct_geometry_create", "cbct_geometry_create_ex", "cbct_set_detector_binning", "cbct_fbs_vcycle", "cbct_fdk_reconstruct",
-    "cbct_fbs_reconstruct_sharded", "cbct_cascade_run", "cbct_set_projector_staging", "cbct_set_mirror_symmetry", "cbct_geometry_destroy", "cbct_geometry_query", "cbct_geometry_coarsen",
+    "cbct_fbs_reconstruct_sharded", "cbct_cascade_run", "cbct_set_projector_staging", "cbct_set_mirror_symmetry", "cbct_set_guard_mode", "cbct_check_guards", "cbct_geometry_destroy", "cbct_geometry_query", "cbct_geometry_coarsen",
     "cbct_forward", "cbct_backproject", "cbct_backproject_eq2", "cbct_set_backprojector", "cbct_tv_prox", "cbct_prolong", "cbct_restrict", "cbct_bin2x2",
     "cbct_energy", "cbct_data_gradient", "cbct_prox_step", "cbct_fbs_reconstruct", "cbct_fbs_reconstruct_until", "cbct_forward_host", "cbct_backproject_host", "cbct_tv_prox_host",
     "cbct_fbs_reconstruct_host", "cbct_profile_enable", "cbct_profile_read", "cbct_launch_count", "cbct_device_bytes", "cbct_last_error",
@@ -68,6 +68,8 @@ def load():
     L.cbct_set_detector_binning.argtypes = [vp, i]
     L.cbct_set_projector_staging.argtypes = [vp, i]
     L.cbct_set_mirror_symmetry.argtypes = [vp, i]
+    L.cbct_set_guard_mode.argtypes = [i]
+    L.cbct_check_guards.argtypes = [vp, C.POINTER(C.c_ulonglong)]
     L.cbct_fbs_vcycle.argtypes = [vp, fp, fp, i, i, i, i, i, i, f, f, f, f, fp, dp, vp]
     L.cbct_fdk_reconstruct.argtypes = [vp, fp, fp, vp]
     L.cbct_fbs_reconstruct_sharded.argtypes = [vp, fp, fp, i, ip, i, f, f, f, f, i, ALLREDUCE_FN, vp, fp, fp, vp]
@@ -113,6 +115,11 @@ def launch_count() -> int:
 
 
 PROFILE_TAGS = ("pad_copy", "forward", "proj_prefix", "backproject", "combine", "tv_sweep", "transfers", "reductions")
+
+
+def set_guard_mode(on: bool):
+    """Place every device buffer allocated from now on between pattern-filled guard regions (Geometry.check_guards)."""
+    _check(load().cbct_set_guard_mode(1 if on else 0))
 
 
 def profile_enable(on: bool):
@@ -224,6 +231,12 @@ class Geometry:
     def set_mirror_symmetry(self, on: bool):
         """Projector / exact backprojector: treat mirrored rays / voxel rows together where the scan is symmetric about z = 0 (True, default)."""
         _check(load().cbct_set_mirror_symmetry(self._h, 1 if on else 0))
+
+    def check_guards(self) -> int:
+        """Pattern bytes around this handle's device buffers that were overwritten (guard mode, see set_guard_mode)."""
+        n = C.c_ulonglong(0)
+        _check(load().cbct_check_guards(self._h, C.byref(n)))
+        return int(n.value)
 
     def set_detector_binning(self, on: bool):
         """Coarse levels bin the detector 2x2 (default) or keep it at full resolution; drops existing coarse levels."""

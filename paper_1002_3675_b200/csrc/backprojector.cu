@@ -382,7 +382,7 @@ static cbct_status launch_gather(cbct_geometry *g, const float *d_scaled, cudaSt
     for (int c = 0; c < 2; ++c) {
         if (g->n_tiles[c] == 0) continue;
         if (g->G_parts_alloc[c] < g->bp_parts) {
-            if (g->G_cls[c]) { CBCT_CUDA(cudaStreamSynchronize(st)); cudaFree(g->G_cls[c]); g->bytes -= g->n_vox() * sizeof(float) * g->G_parts_alloc[c]; g->G_cls[c] = nullptr; }
+            if (g->G_cls[c]) { CBCT_CUDA(cudaStreamSynchronize(st)); cbct_dev_free(g, g->G_cls[c]); g->bytes -= g->n_vox() * sizeof(float) * g->G_parts_alloc[c]; g->G_cls[c] = nullptr; }
             CBCT_TRY(ensure(g, &g->G_cls[c], g->n_vox() * g->bp_parts));
             g->G_parts_alloc[c] = g->bp_parts;
         }

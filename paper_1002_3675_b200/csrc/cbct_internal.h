@@ -96,6 +96,8 @@ struct cbct_geometry {
     double *h_red = nullptr;                  // pinned host mirror of red_out
     float *host_stage_vol = nullptr, *host_stage_proj = nullptr, *host_stage_vol2 = nullptr;  // device staging for *_host
     unsigned long long bytes = 0;
+    struct Guarded { void *ptr; size_t bytes, padded; };
+    std::vector<Guarded> guarded;             // buffers allocated in guard mode (cbct_set_guard_mode): user pointer, sizes
 
     int bp_parts = 1, G_parts_alloc[2] = {0, 0};   // gather: angle parts per column chunk (small volumes), partial volumes allocated
     int bp_mode = 0;                          // step 1 of A1: 0 exact transpose, 1 eq. 2 (cbct_set_backprojector)
@@ -156,6 +158,7 @@ struct ProfileScope {
 // ---- scratch ------------------------------------------------------------------------------
 // zero = true clears the new buffer with cudaMemsetAsync on `st`, the stream of the first kernel that will use it
 cbct_status cbct_dev_alloc(cbct_geometry *g, void **p, size_t bytes, bool zero, cudaStream_t st);
+void cbct_dev_free(cbct_geometry *g, void *p);
 template <typename T>
 inline cbct_status ensure(cbct_geometry *g, T **p, size_t count)
 {

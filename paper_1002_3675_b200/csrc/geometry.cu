@@ -21,19 +21,76 @@ void cbct_set_error(const char *fmt, ...)
 extern "C" const char *cbct_last_error(void) { return t_err; }
 extern "C" unsigned long long cbct_launch_count(void) { return g_cbct_launches.load(); }
 
+// Guard mode (cbct_set_guard_mode): every device buffer a handle allocates from then on sits between two kGuard-byte
+// regions filled with a pattern; cbct_check_guards counts the pattern bytes that changed.  It stands in for compute-sanitizer's
+// memcheck, which this pool does not allow: an out-of-bounds WRITE of any kernel into library-owned memory shows up there.
+static constexpr size_t kGuard = 4096;
+static constexpr unsigned char kGuardByte = 0xA5;
+static std::atomic<int> g_guard_mode{0};
+
+extern "C" cbct_status cbct_set_guard_mode(int on)
+{
+    g_guard_mode.store(on != 0);
+    return CBCT_OK;
+}
+
 cbct_status cbct_dev_alloc(cbct_geometry *g, void **p, size_t bytes, bool zero, cudaStream_t st)
 {
-    cudaError_t e = cudaMalloc(p, bytes);
+    const bool guard = g_guard_mode.load() != 0;
+    const size_t padded = (bytes + 255) / 256 * 256;            // the rear guard starts on a 256-byte boundary behind the buffer
+    void *base = nullptr;
+    cudaError_t e = cudaMalloc(&base, guard ? padded + 2 * kGuard : bytes);
     if (e != cudaSuccess) {
         *p = nullptr;
         cudaGetLastError();
         cbct_set_error("cudaMalloc(%zu bytes) failed: %s", bytes, cudaGetErrorString(e));
         return CBCT_ERR_ALLOC;
     }
+    if (guard) {
+        // whole allocation patterned (so the slack up to `padded` is guarded too), then waited for: debug mode
+        CBCT_CUDA(cudaMemset(base, kGuardByte, padded + 2 * kGuard));
+        CBCT_CUDA(cudaDeviceSynchronize());
+        *p = static_cast<char *>(base) + kGuard;
+        g->guarded.push_back({*p, bytes, padded});
+    } else {
+        *p = base;
+    }
     // zero-fill ON THE CALLER'S STREAM: the first kernel that touches the buffer is launched on it right afterwards,
     // and nothing orders the legacy default stream against a non-blocking stream (PyTorch's side streams)
     if (zero) CBCT_CUDA(cudaMemsetAsync(*p, 0, bytes, st));
     g->bytes += bytes;
+    return CBCT_OK;
+}
+
+void cbct_dev_free(cbct_geometry *g, void *p)
+{
+    if (!p) return;
+    for (size_t n = 0; n < g->guarded.size(); ++n)
+        if (g->guarded[n].ptr == p) {
+            cudaFree(static_cast<char *>(p) - kGuard);
+            g->guarded.erase(g->guarded.begin() + n);
+            return;
+        }
+    cudaFree(p);
+}
+
+extern "C" cbct_status cbct_check_guards(const cbct_geometry *gc, unsigned long long *h_bad_bytes)
+{
+    if (!gc || !h_bad_bytes) { cbct_set_error("cbct_check_guards: NULL argument"); return CBCT_ERR_INVALID_ARG; }
+    *h_bad_bytes = 0;
+    CBCT_CUDA(cudaDeviceSynchronize());
+    std::vector<unsigned char> h;
+    for (const cbct_geometry *g = gc; g; g = g->coarse)
+        for (const auto &b : g->guarded) {
+            const char *user = static_cast<const char *>(b.ptr);
+            // front guard, then everything from the end of the user's bytes to the end of the rear guard
+            const struct { const char *at; size_t n; } spans[2] = {{user - kGuard, kGuard}, {user + b.bytes, b.padded - b.bytes + kGuard}};
+            for (const auto &sp : spans) {
+                h.resize(sp.n);
+                CBCT_CUDA(cudaMemcpy(h.data(), sp.at, sp.n, cudaMemcpyDeviceToHost));
+                for (unsigned char c : h) *h_bad_bytes += c != kGuardByte;
+            }
+        }
     return CBCT_OK;
 }
 
@@ -45,8 +102,7 @@ static void free_handle(cbct_geometry *g)
                     g->d_angle_has[0], g->d_angle_has[1], g->vol_pad[0], g->vol_pad[1], g->proj_tmp, g->proj_prefix,
                     g->G_cls[0], g->G_cls[1], g->vol_a, g->vol_b, g->vol_c, g->vol_f, g->Y_level, g->vc_tau, g->vc_f0, g->vc_d, g->vc_e, g->fdk_q, g->fdk_hk,
                     g->red_partial, g->red_out, g->host_stage_vol, g->host_stage_proj, g->host_stage_vol2};
-    for (void *p : ptrs)
-        if (p) cudaFree(p);
+    for (void *p : ptrs) cbct_dev_free(g, p);
     if (g->h_red) cudaFreeHost(g->h_red);
     if (g->graph_stream) cudaStreamDestroy(g->graph_stream);
     delete g;
