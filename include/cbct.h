@@ -317,7 +317,9 @@ cbct_status cbct_cascade_run(const cbct_cascade_ops *ops, int n_levels, const in
 /*
  * Host-buffer variants (end-to-end path): same operations with HOST pointers; each call copies its
  * inputs host->device and its result device->host on `cuda_stream` (use pinned host memory for
- * full copy speed) and returns after synchronising the stream.
+ * full copy speed) and returns after synchronising the stream.  cbct_fbs_reconstruct_host uploads h_Y from an internal
+ * second stream, behind h_f0 on the bus and beside the cascade's first kernels (those that do not need Y); its result equals
+ * cbct_fbs_reconstruct on the same data bit for bit.
  */
 cbct_status cbct_forward_host(const cbct_geometry *g, const float *h_vol, float *h_proj, void *cuda_stream);
 cbct_status cbct_backproject_host(const cbct_geometry *g, const float *h_proj, float *h_vol, void *cuda_stream);

@@ -196,7 +196,7 @@ extern "C" cbct_status cbct_prox_step(const cbct_geometry *gc, const float *d_f,
 // tau != nullptr (FAS coarse problems, vcycle.cu): the linear term -<tau, f> joins the gradient of step 1, gv = f - c G + tau / beta.
 cbct_status op_fbs_level(cbct_geometry *g, const float *d_Y, float *f, int n_outer, int n_inner, float step,
                          float mu, float eps, float omega, double *trace, float rel_tol, int *iters, const float *tau,
-                         cudaStream_t st)
+                         cudaStream_t st, const std::function<cbct_status()> *y_gate)
 {
     if (rel_tol > 0.f) {
         CBCT_TRY(ensure(g, &g->vol_c, g->n_vox()));
@@ -209,18 +209,30 @@ cbct_status op_fbs_level(cbct_geometry *g, const float *d_Y, float *f, int n_out
     const float beta = mu / step;
     const float c = (float)(2.0 * (double)step * (double)g->n_vox() / ((double)g->na * g->nu * g->nv));
     // one outer iteration (steps 1-3 of A1) on stream s: the same launches with the same arguments every iteration
-    auto iteration = [&](cudaStream_t s) -> cbct_status {
+    // gate != nullptr (host-buffer path, first iteration only): Y is still on its way to the device, so the projection runs
+    // without the fused residual, then the gate waits for Y (and bins it for the coarse levels), then a2 runs on its own
+    auto iteration = [&](cudaStream_t s, const std::function<cbct_status()> *gate) -> cbct_status {
         CBCT_TRY(op_pad_copies(g, f, s));
         if (g->bp_mode == CBCT_BACKPROJECTOR_EQ2) {
             // the paper's step 1 (P:87 with eq. 2): dE2/df = (2/(N_theta A)) B r, so gv = f - c (dV/(du dv)) B r
             const float c2 = (float)((double)c * (g->hx * g->hy * g->hz) / (g->du * g->dv));
-            CBCT_TRY(op_forward_padded(g, g->proj_tmp, d_Y, 2, s));      // P f - Y              a1+a2
+            if (gate) {
+                CBCT_TRY(op_forward_padded(g, g->proj_tmp, nullptr, 0, s));
+                CBCT_TRY((*gate)());
+                CBCT_TRY(op_residual(g, g->proj_tmp, d_Y, 2, s));
+            } else
+                CBCT_TRY(op_forward_padded(g, g->proj_tmp, d_Y, 2, s));  // P f - Y              a1+a2
             CBCT_TRY(op_backproject_eq2(g, g->proj_tmp, f, c2, n_inner == 0 && !tau, g->vol_a, s));   // a3 (eq. 2) + a4 (+ a6)
             if (tau) CBCT_TRY(op_axpy_clamp(g, g->vol_a, tau, -1.f / beta, n_inner == 0, g->vol_a, s));
             if (n_inner == 0) CBCT_CUDA(cudaMemcpyAsync(f, g->vol_a, g->n_vox() * sizeof(float), cudaMemcpyDeviceToDevice, s));
             else CBCT_TRY(tv_inner(g, g->vol_a, g->vol_a, f, beta, eps, omega, n_inner, 1, s));
         } else {
-            CBCT_TRY(op_forward_padded(g, g->proj_tmp, d_Y, 1, s));          // l (P f - Y)          a1+a2
+            if (gate) {
+                CBCT_TRY(op_forward_padded(g, g->proj_tmp, nullptr, 0, s));
+                CBCT_TRY((*gate)());
+                CBCT_TRY(op_residual(g, g->proj_tmp, d_Y, 1, s));
+            } else
+                CBCT_TRY(op_forward_padded(g, g->proj_tmp, d_Y, 1, s));      // l (P f - Y)          a1+a2
             CBCT_TRY(op_backproject_prefix(g, g->proj_tmp, 0, nullptr, s));
             CBCT_TRY(op_backproject_gather(g, g->proj_tmp, s));              // P^T (P f - Y)        a3
             CBCT_TRY(op_combine(g, f, c, n_inner == 0 && !tau, g->vol_a, s));    // gv = f - c G (a4), clamped (a6) if nothing follows
@@ -234,7 +246,7 @@ cbct_status op_fbs_level(cbct_geometry *g, const float *d_Y, float *f, int n_out
     // every allocation) the iteration is captured once into a CUDA graph on an internal stream and replayed on the caller's.
     // Any failure to capture falls back to eager launches.
     cudaGraphExec_t gexec = nullptr;
-    const bool want_graph = !trace && rel_tol == 0.f && !cbct_profile_is_on() && n_outer >= 6 && g->n_vox() <= ((size_t)1 << 20);
+    const bool want_graph = !trace && rel_tol == 0.f && !y_gate && !cbct_profile_is_on() && n_outer >= 6 && g->n_vox() <= ((size_t)1 << 20);
     for (int it = 0; it < n_outer; ++it) {
         if (rel_tol > 0.f) CBCT_CUDA(cudaMemcpyAsync(g->vol_c, f, g->n_vox() * sizeof(float), cudaMemcpyDeviceToDevice, st));
         if (want_graph && it == 1 && !gexec) {
@@ -242,7 +254,7 @@ cbct_status op_fbs_level(cbct_geometry *g, const float *d_Y, float *f, int n_out
             cudaGraph_t graph = nullptr;
             if (g->graph_stream && cudaStreamBeginCapture(g->graph_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
                 const unsigned long long n0 = g_cbct_launches.load();
-                const cbct_status cs = iteration(g->graph_stream);           // recorded, not run
+                const cbct_status cs = iteration(g->graph_stream, nullptr);  // recorded, not run
                 g_cbct_launches.store(n0);
                 const cudaError_t ce = cudaStreamEndCapture(g->graph_stream, &graph);
                 if (cs != CBCT_OK || ce != cudaSuccess || !graph || cudaGraphInstantiate(&gexec, graph, 0) != cudaSuccess) gexec = nullptr;
@@ -255,7 +267,7 @@ cbct_status op_fbs_level(cbct_geometry *g, const float *d_Y, float *f, int n_out
             g_cbct_launches += g->launches_per_iteration;
         } else {
             const unsigned long long n0 = g_cbct_launches.load();
-            CBCT_TRY(iteration(st));
+            CBCT_TRY(iteration(st, it == 0 ? y_gate : nullptr));
             g->launches_per_iteration = g_cbct_launches.load() - n0;
         }
         if (trace) {
@@ -278,7 +290,8 @@ cbct_status op_fbs_level(cbct_geometry *g, const float *d_Y, float *f, int n_out
 
 static cbct_status fbs_cascade(const cbct_geometry *gc, const float *d_Y, const float *d_f0, int n_levels,
                                const int *n_outer, int n_inner, float step, float mu, float eps, float omega,
-                               float *d_f_out, double *trace, float rel_tol, int *iters_per_level, void *stream)
+                               float *d_f_out, double *trace, float rel_tol, int *iters_per_level, void *stream,
+                               cudaEvent_t y_ready = nullptr)
 {
     REQUIRE(gc && d_Y && d_f_out && n_outer, "cbct_fbs_reconstruct: NULL argument");
     REQUIRE(n_levels >= 1 && n_levels <= 16 && n_inner >= 0, "cbct_fbs_reconstruct: n_levels < 1 (or > 16) or n_tv_inner < 0");
@@ -293,14 +306,24 @@ static cbct_status fbs_cascade(const cbct_geometry *gc, const float *d_Y, const 
         CBCT_TRY(cbct_geometry_coarsen(lev[l - 1], &lev[l], nullptr));
     }
 
-    // data per level: level 0 uses d_Y, coarser levels their own binned copy
+    // data per level: level 0 uses d_Y, coarser levels their own binned copy.  y_ready (host-buffer path): d_Y is still being
+    // uploaded on another stream; everything that does not need it (the restriction of f0, the padded copies and the first
+    // projection of the coarsest level) runs first, then `gate` waits for the upload and bins
     std::vector<const float *> Y(n_levels);
     Y[0] = d_Y;
     for (int l = 1; l < n_levels; ++l) {
         CBCT_TRY(ensure(lev[l], &lev[l]->Y_level, lev[l]->n_proj()));
-        CBCT_TRY(op_bin2x2(lev[l - 1], Y[l - 1], lev[l]->Y_level, st));
         Y[l] = lev[l]->Y_level;
     }
+    bool y_here = false;
+    const std::function<cbct_status()> gate = [&]() -> cbct_status {
+        if (y_here) return CBCT_OK;
+        y_here = true;
+        if (y_ready) CBCT_CUDA(cudaStreamWaitEvent(st, y_ready, 0));
+        for (int l = 1; l < n_levels; ++l) CBCT_TRY(op_bin2x2(lev[l - 1], Y[l - 1], lev[l]->Y_level, st));
+        return CBCT_OK;
+    };
+    if (!y_ready) CBCT_TRY(gate());
     // current iterate per level lives in vol_f of that level (level 0: the caller's output buffer)
     std::vector<float *> F(n_levels);
     F[0] = d_f_out;
@@ -321,7 +344,8 @@ static cbct_status fbs_cascade(const cbct_geometry *gc, const float *d_Y, const 
     for (int l = L; l >= 0; --l) {
         const int n = n_outer[L - l];
         CBCT_TRY(op_fbs_level(lev[l], Y[l], F[l], n, n_inner, step, mu, eps, omega, trace ? trace + done : nullptr, rel_tol,
-                              iters_per_level ? iters_per_level + (L - l) : nullptr, nullptr, st));
+                              iters_per_level ? iters_per_level + (L - l) : nullptr, nullptr, st, y_here ? nullptr : &gate));
+        CBCT_TRY(gate());                                        // a level with no iterations has not opened it
         done += n;
         if (l > 0) CBCT_TRY(op_prolong(lev[l - 1], F[l], F[l - 1], st));
     }
@@ -399,11 +423,27 @@ extern "C" cbct_status cbct_fbs_reconstruct_host(const cbct_geometry *gc, const 
     cudaStream_t st = (cudaStream_t)stream;
     CBCT_TRY(ensure(g, &g->host_stage_vol, g->n_vox()));
     CBCT_TRY(ensure(g, &g->host_stage_proj, g->n_proj()));
-    CBCT_CUDA(cudaMemcpyAsync(g->host_stage_proj, h_Y, g->n_proj() * sizeof(float), cudaMemcpyHostToDevice, st));
+    if (!g->copy_stream) {
+        CBCT_CUDA(cudaStreamCreateWithFlags(&g->copy_stream, cudaStreamNonBlocking));
+        CBCT_CUDA(cudaEventCreateWithFlags(&g->ev_f0, cudaEventDisableTiming));
+        CBCT_CUDA(cudaEventCreateWithFlags(&g->ev_Y, cudaEventDisableTiming));
+    }
+    // The cascade needs all of f0 before its first kernel (the coarsest level starts from the restricted f0), Y only when the
+    // first projection of that level is done: f0 goes first, on the caller's stream; Y follows it on the bus from a second
+    // stream (behind an event, so that the two uploads do not share the bandwidth) while the restriction, the padded copies and
+    // that projection run; the cascade waits for Y where it first needs it.  The download of f cannot be hidden.
     if (h_f0)
         CBCT_CUDA(cudaMemcpyAsync(g->host_stage_vol, h_f0, g->n_vox() * sizeof(float), cudaMemcpyHostToDevice, st));
-    CBCT_TRY(cbct_fbs_reconstruct(g, g->host_stage_proj, h_f0 ? g->host_stage_vol : nullptr, n_levels, n_outer, n_inner,
-                                  step, mu, eps, omega, g->host_stage_vol, trace, stream));
+    CBCT_CUDA(cudaEventRecord(g->ev_f0, st));
+    CBCT_CUDA(cudaStreamWaitEvent(g->copy_stream, g->ev_f0, 0));
+    CBCT_CUDA(cudaMemcpyAsync(g->host_stage_proj, h_Y, g->n_proj() * sizeof(float), cudaMemcpyHostToDevice, g->copy_stream));
+    CBCT_CUDA(cudaEventRecord(g->ev_Y, g->copy_stream));
+    const cbct_status rc = fbs_cascade(g, g->host_stage_proj, h_f0 ? g->host_stage_vol : nullptr, n_levels, n_outer, n_inner, step,
+                                       mu, eps, omega, g->host_stage_vol, trace, 0.f, nullptr, stream, g->ev_Y);
+    if (rc != CBCT_OK) {                                         // never leave the upload running into a buffer the caller may free
+        cudaStreamSynchronize(g->copy_stream);
+        return rc;
+    }
     CBCT_CUDA(cudaMemcpyAsync(h_f_out, g->host_stage_vol, g->n_vox() * sizeof(float), cudaMemcpyDeviceToHost, st));
     CBCT_CUDA(cudaStreamSynchronize(st));
     return CBCT_OK;

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include <atomic>
+#include <functional>
 
 #include <cstdint>
 #include <cmath>
@@ -106,6 +107,8 @@ struct cbct_geometry {
     int fw_bj[2] = {0, 0}, fw_bk[2] = {0, 0};  // brick spans per class (0 = not computed yet)
     int bin_detector = 1;                     // coarse levels bin the detector 2x2 (O6) or keep it at full resolution (Q20)
 
+    cudaStream_t copy_stream = nullptr;       // host-buffer path: the upload of Y runs here, beside the first kernels (api.cu)
+    cudaEvent_t ev_f0 = nullptr, ev_Y = nullptr;
     cudaStream_t graph_stream = nullptr;      // internal stream the outer iteration of a small volume is captured on (api.cu)
     unsigned long long launches_per_iteration = 0;   // kernels one outer iteration launches (counted on an eager one)
 
@@ -181,6 +184,8 @@ inline size_t pad_elems(const cbct_geometry *g, int c)
 cbct_status op_pad_copies(cbct_geometry *g, const float *d_vol, cudaStream_t st);
 // mode 0: out = P f ; mode 1: out = l * (P f - Y)  (scaled residual for the gather) ; mode 2: out = P f - Y
 cbct_status op_forward_padded(cbct_geometry *g, float *d_out, const float *d_Y, int mode, cudaStream_t st);
+// q (= P f from mode 0) -> l (q - Y) (mode 1) or q - Y (mode 2), in place: a2 on its own, bit-identical to the fused store
+cbct_status op_residual(cbct_geometry *g, float *d_q, const float *d_Y, int mode, cudaStream_t st);
 cbct_status op_forward_padded_tma(cbct_geometry *g, float *d_out, const float *d_Y, int mode, cudaStream_t st, int *done);   // projector_tma.cu
 // backprojector.cu : gathers of the (already l-scaled) projections into G_cls[0], G_cls[1].
 // op_backproject_prefix builds the prefix sums along v that the gather reads (scale != 0: of l * d_in,
@@ -209,7 +214,8 @@ cbct_status op_sumsq_diff(cbct_geometry *g, const float *a, const float *b, size
 cbct_status op_tv_grad(cbct_geometry *g, const float *f, float eps, float *out, cudaStream_t st);   // tv.cu: out = grad TV_eps(f)
 // api.cu: one level of A1 (tau: optional FAS term), the data gradient P^T (P f - Y) (or eq. 2's), E_eps (synchronises)
 cbct_status op_fbs_level(cbct_geometry *g, const float *d_Y, float *f, int n_outer, int n_inner, float step, float mu, float eps,
-                         float omega, double *trace, float rel_tol, int *iters, const float *tau, cudaStream_t st);
+                         float omega, double *trace, float rel_tol, int *iters, const float *tau, cudaStream_t st,
+                         const std::function<cbct_status()> *y_gate = nullptr);   // y_gate: see api.cu (host-buffer path)
 cbct_status op_data_gradient(cbct_geometry *g, const float *d_f, const float *d_Y, float *d_G, cudaStream_t st);
 cbct_status op_energy(cbct_geometry *g, const float *d_f, const float *d_Y, float mu, float eps, double *out3, cudaStream_t st);
 cbct_status op_axpy_clamp(cbct_geometry *g, const float *f, const float *G, float c, int clamp, float *out, cudaStream_t st);

@@ -105,6 +105,9 @@ static void free_handle(cbct_geometry *g)
     for (void *p : ptrs) cbct_dev_free(g, p);
     if (g->h_red) cudaFreeHost(g->h_red);
     if (g->graph_stream) cudaStreamDestroy(g->graph_stream);
+    if (g->copy_stream) cudaStreamDestroy(g->copy_stream);
+    if (g->ev_f0) cudaEventDestroy(g->ev_f0);
+    if (g->ev_Y) cudaEventDestroy(g->ev_Y);
     delete g;
 }
 

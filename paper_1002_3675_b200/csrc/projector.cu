@@ -189,13 +189,37 @@ forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, c
 #pragma unroll
             for (int m = 0; m < (MIRROR ? 2 : 1); ++m) {
                 const size_t o = ((size_t)a * d.nv + (m ? d.nv - 1 - v : v)) * d.nu + u;
-                float val = len * (m ? accM[MIRROR ? q : 0] : acc[q]);
-                if (mode == 1) val = len * (val - __ldg(Y + o));
-                else if (mode == 2) val -= __ldg(Y + o);
+                // uncontracted (no FMA across the subtraction), so that op_residual applied to a stored mode-0 value is bit-identical
+                float val = __fmul_rn(len, m ? accM[MIRROR ? q : 0] : acc[q]);
+                if (mode == 1) val = __fmul_rn(len, __fsub_rn(val, __ldg(Y + o)));
+                else if (mode == 2) val = __fsub_rn(val, __ldg(Y + o));
                 out[o] = val;
             }
         }
     }
+}
+
+// a2 alone: turns a plain projection q = P f (mode 0 of the march) into the residual the march's mode 1 / mode 2 would have
+// stored, with the very same operations (val = len * acc was stored; here len * (val - Y) or val - Y), so the result is bit
+// for bit the fused one.  Used by the host-buffer path, whose first projection starts before Y has arrived on the device.
+__global__ void __launch_bounds__(256) residual_kernel(const DevGeom d, float *__restrict__ q, const float *__restrict__ Y, const int mode)
+{
+    const int u = blockIdx.x * blockDim.x + threadIdx.x, v = blockIdx.y, a = blockIdx.z;
+    if (u >= d.nu) return;
+    const size_t o = ((size_t)a * d.nv + v) * d.nu + u;
+    float val = q[o];
+    if (mode == 1) val = __fmul_rn(chord_scale(load_ray(d, a, u), __ldg(d.dz_mm + v)), __fsub_rn(val, __ldg(Y + o)));
+    else val = __fsub_rn(val, __ldg(Y + o));
+    q[o] = val;
+}
+
+cbct_status op_residual(cbct_geometry *g, float *d_q, const float *d_Y, int mode, cudaStream_t st)
+{
+    ProfileScope ps(1, st);
+    dim3 grid((g->nu + 255) / 256, g->nv, g->na);
+    residual_kernel<<<grid, 256, 0, st>>>(g->dev, d_q, d_Y, mode);
+    CBCT_LAUNCH_CHECK();
+    return CBCT_OK;
 }
 
 // the scan is its own mirror image about the central plane: even slice and detector-row counts, detector centred in v

@@ -215,9 +215,9 @@ forward_tma_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tile
         if (v < d.nv) {
             const float len = chord_scale(ro, __ldg(d.dz_mm + v));
             const size_t o = ((size_t)a * d.nv + v) * d.nu + u;
-            float val = active ? len * acc[q] : 0.f;
-            if (mode == 1) val = len * (val - __ldg(Y + o));
-            else if (mode == 2) val -= __ldg(Y + o);
+            float val = active ? __fmul_rn(len, acc[q]) : 0.f;           // uncontracted, as in projector.cu
+            if (mode == 1) val = __fmul_rn(len, __fsub_rn(val, __ldg(Y + o)));
+            else if (mode == 2) val = __fsub_rn(val, __ldg(Y + o));
             out[o] = val;
         }
     }

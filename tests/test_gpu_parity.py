@@ -363,6 +363,21 @@ def test_host_entry_points(cuda_lib, dev):
     u = vol.copy()
     cb.tv_prox_host(G, vol, u, 40.0, 1e-3, 1.0, 3)
     assert rel(u, o.tv_prox(g, vol.astype(np.float64), vol.astype(np.float64), 40.0, 1e-3, 1.0, 3)) <= TOL_OP
+    # the host-buffer cascade uploads Y beside its first kernels (projection without the fused residual, then a2 on its own):
+    # bit for bit the device-resident cascade, with and without a start volume, with either backprojector, also on a side stream
+    import torch
+    Y = f32(0.9 * q + 0.01)
+    st = torch.cuda.Stream(device=dev)
+    for mode in (cb.BACKPROJECTOR_EXACT, cb.BACKPROJECTOR_EQ2):
+        cb.set_backprojector(G, mode)
+        for f0 in (None, f32(0.5 * vol)):
+            for stream in (None, st):
+                d_f = torch.empty(G.vol_shape, device=dev)
+                cb.fbs_reconstruct(G, to_dev(Y, dev), None if f0 is None else to_dev(f0, dev), 2, [2, 3], 3, 1e-4, 1.0, 1e-4, 1.0, d_f)
+                torch.cuda.synchronize()
+                h_f = np.empty(g.vol_shape, dtype=np.float32)
+                cb.fbs_reconstruct_host(G, Y, f0, 2, [2, 3], 3, 1e-4, 1.0, 1e-4, 1.0, h_f, stream=stream)
+                assert np.array_equal(h_f, d_f.cpu().numpy())
     G.close()
 
 
