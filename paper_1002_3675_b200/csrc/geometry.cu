@@ -264,8 +264,16 @@ static cbct_status build_tables(cbct_geometry *g)
     CBCT_TRY(upload(g, &g->d_zeta, zeta));
     CBCT_TRY(upload(g, &g->d_inv_zeta, inv_zeta));
     CBCT_TRY(upload(g, &g->d_dz, dz));
+    // the angle list closed under + 180 degrees, second half in the order of the first?
+    g->twin_ok = na % 2 == 0 && na >= 2;
+    for (int a = 0; g->twin_ok && a < na / 2; ++a) {
+        const double dlt = std::remainder(g->angles[a + na / 2] - g->angles[a] - 3.14159265358979323846, 2.0 * 3.14159265358979323846);
+        if (std::fabs(dlt) > 1e-12) g->twin_ok = false;
+    }
     for (int c = 0; c < 2; ++c) {
         g->n_tiles[c] = (int)tiles[c].size();
+        g->n_tiles_half[c] = 0;
+        for (const int2 &t : tiles[c]) g->n_tiles_half[c] += t.x < na / 2;
         CBCT_TRY(upload(g, &g->d_tiles[c], tiles[c]));
         CBCT_TRY(upload(g, &g->d_angle_has[c], g->h_angle_has[c]));
     }

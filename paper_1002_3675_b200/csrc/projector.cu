@@ -63,7 +63,12 @@ cbct_status op_pad_copies(cbct_geometry *g, const float *d_vol, cudaStream_t st)
 // (u, nv-1-v) is then the mirror image of ray (u, v): same x-y traversal, same crossing positions b, z rows nz-1-k.  A thread
 // marches V rays of the UPPER half of the detector (v >= nv/2) together with their V mirror images, so the z arithmetic of a
 // slab (entry position, b, the row advance and its clamps) is done once for two rays.
-template <int V, int WARPS, bool MIRROR>
+// TWIN (with MIRROR): the angle list is closed under theta -> theta + 180 degrees (angle a + na/2 = angle a + pi).  Turning
+// the whole scan by 180 degrees about the rotation axis maps ray (a, u, v) onto ray (a + na/2, u, v) and voxel (i, j, k) onto
+// (nx-1-i, ny-1-j, k): the twin ray has the same slabs, splits a and b and chord fractions, met in the point-reflected
+// voxels, i.e. at padded offset (nmaj-1) row_stride + nmin-2 minus the ray's own, with the two minor rows swapped.  A thread
+// then marches V rays, their z-mirror images and the twins of both: 4 V rays from one evaluation of all the ray arithmetic.
+template <int V, int WARPS, bool MIRROR, bool TWIN = false>
 __global__ void __launch_bounds__(32 * WARPS)
 forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, const float *__restrict__ vol,
                float *__restrict__ out, const float *__restrict__ Y, const int mode)
@@ -98,12 +103,17 @@ forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, c
     const int lo_w = __reduce_min_sync(0xffffffffu, active ? ilo : 0x7fffffff);
     const int hi_w = __reduce_max_sync(0xffffffffu, active ? ihi : -1);
 
-    float acc[V], accM[MIRROR ? V : 1];
+    static_assert(!TWIN || MIRROR, "the twin march is built on the mirrored one");
+    float acc[V], accM[MIRROR ? V : 1], accT[TWIN ? V : 1], accMT[TWIN ? V : 1];
 #pragma unroll
     for (int q = 0; q < V; ++q) acc[q] = 0.f;
     if constexpr (MIRROR) {
 #pragma unroll
         for (int q = 0; q < V; ++q) accM[q] = 0.f;
+    }
+    if constexpr (TWIN) {
+#pragma unroll
+        for (int q = 0; q < V; ++q) accT[q] = accMT[q] = 0.f;
     }
 
     if (lo_w < hi_w) {
@@ -114,6 +124,8 @@ forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, c
         const int pstride = (int)cg.plane_stride;
         // MIRROR: padded row of the mirror image = (nz - 1 + 2 kPadK) - padded row (the clamp range is symmetric)
         const int row_top = (d.nz - 1 + 2 * kPadK) * pstride;
+        // TWIN: offset of the point-reflected row pair inside a padded plane = off_top - (the ray's own offset)
+        const int off_top = (cg.nmaj - 1) * cg.row_stride + cg.nmin - 2;
         const float e0 = (float)(lo_w - cg.ioff);
         const float T0 = fmaf(e0, r.dt, r.tc);
 #pragma unroll
@@ -154,6 +166,14 @@ forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, c
                     accM[q] = fmaf(wlo, __ldg(pm), accM[q]);
                     accM[q] = fmaf(whi, __ldg(pm + 1), accM[q]);
                 }
+                if constexpr (TWIN) {                          // reflected rows: [0] is the twin of p[1], [1] the twin of p[0]
+                    const float *pt = base + (rowoff[q] + (off_top - off_i));
+                    accT[q] = fmaf(whi, __ldg(pt), accT[q]);
+                    accT[q] = fmaf(wlo, __ldg(pt + 1), accT[q]);
+                    const float *pmt = base + ((row_top - rowoff[q]) + (off_top - off_i));
+                    accMT[q] = fmaf(whi, __ldg(pmt), accMT[q]);
+                    accMT[q] = fmaf(wlo, __ldg(pmt + 1), accMT[q]);
+                }
             }
             // Pass 2: a ray that crosses a z plane inside the slab (b < 1) moves its exit-row fractions
             // a - min(a,b) (row ja) and 1 - max(a,b) (row ja+dir) to the next z row, and continues there.
@@ -174,6 +194,15 @@ forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, c
                         accM[q] = fmaf(c_lo, __ldg(pm1) - __ldg(pm), accM[q]);
                         accM[q] = fmaf(c_hi, __ldg(pm1 + 1) - __ldg(pm + 1), accM[q]);
                     }
+                    if constexpr (TWIN) {
+                        const int offt = off_top - off_i;
+                        const float *pt = base + (rowoff[q] + offt), *pt1 = base + (rowoff1 + offt);
+                        accT[q] = fmaf(c_hi, __ldg(pt1) - __ldg(pt), accT[q]);
+                        accT[q] = fmaf(c_lo, __ldg(pt1 + 1) - __ldg(pt + 1), accT[q]);
+                        const float *pmt = base + ((row_top - rowoff[q]) + offt), *pmt1 = base + ((row_top - rowoff1) + offt);
+                        accMT[q] = fmaf(c_hi, __ldg(pmt1) - __ldg(pmt), accMT[q]);
+                        accMT[q] = fmaf(c_lo, __ldg(pmt1 + 1) - __ldg(pmt + 1), accMT[q]);
+                    }
                     zbnd[q] += zs;
                     rowoff[q] = rowoff1;
                 }
@@ -187,10 +216,12 @@ forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, c
         if (v < d.nv) {
             const float len = chord_scale(r, __ldg(d.dz_mm + v));
 #pragma unroll
-            for (int m = 0; m < (MIRROR ? 2 : 1); ++m) {
-                const size_t o = ((size_t)a * d.nv + (m ? d.nv - 1 - v : v)) * d.nu + u;
+            for (int m = 0; m < (TWIN ? 4 : MIRROR ? 2 : 1); ++m) {          // the ray, its z-mirror image, the twins of both
+                const int aa = (m & 2) ? a + d.na / 2 : a, vv = (m & 1) ? d.nv - 1 - v : v;
+                const size_t o = ((size_t)aa * d.nv + vv) * d.nu + u;
+                const float ac = m == 0 ? acc[q] : m == 1 ? accM[MIRROR ? q : 0] : m == 2 ? accT[TWIN ? q : 0] : accMT[TWIN ? q : 0];
                 // uncontracted (no FMA across the subtraction), so that op_residual applied to a stored mode-0 value is bit-identical
-                float val = __fmul_rn(len, m ? accM[MIRROR ? q : 0] : acc[q]);
+                float val = __fmul_rn(len, ac);
                 if (mode == 1) val = __fmul_rn(len, __fsub_rn(val, __ldg(Y + o)));
                 else if (mode == 2) val = __fsub_rn(val, __ldg(Y + o));
                 out[o] = val;
@@ -238,6 +269,9 @@ cbct_status op_forward_padded(cbct_geometry *g, float *d_out, const float *d_Y, 
 #ifndef CBCT_FW_VM
 #define CBCT_FW_VM 3
 #endif
+#ifndef CBCT_FW_VT
+#define CBCT_FW_VT 2
+#endif
     constexpr int V = CBCT_FW_V, WARPS = CBCT_FW_WARPS;
     if (g->fw_staged) {
         int done = 0;
@@ -250,7 +284,12 @@ cbct_status op_forward_padded(cbct_geometry *g, float *d_out, const float *d_Y, 
     const bool mirror = march_is_mirrored(g);
     for (int c = 0; c < 2; ++c) {
         if (g->n_tiles[c] == 0) continue;
-        if (mirror) {
+        if (mirror && g->twin_ok) {
+            constexpr int VT = CBCT_FW_VT;                    // ray quadruples per thread; only the tiles of the first half turn
+            dim3 grid(g->n_tiles_half[c], (g->nv / 2 + VT * WARPS - 1) / (VT * WARPS)), block(32, WARPS);
+            if (grid.x > 0)
+                forward_kernel<VT, WARPS, true, true><<<grid, block, 0, st>>>(g->dev, c, g->d_tiles[c], g->vol_pad[c], d_out, d_Y, mode);
+        } else if (mirror) {
             constexpr int VM = CBCT_FW_VM;                    // ray pairs per thread
             dim3 grid(g->n_tiles[c], (g->nv / 2 + VM * WARPS - 1) / (VM * WARPS)), block(32, WARPS);
             forward_kernel<VM, WARPS, true><<<grid, block, 0, st>>>(g->dev, c, g->d_tiles[c], g->vol_pad[c], d_out, d_Y, mode);

@@ -72,6 +72,12 @@ GEOMS = {
     # odd nv with even nz: the central detector row lies exactly in the voxel plane k = nz/2 (reading Q15: it belongs to the
     # row above); 40 detector rows per slice, so the run bounds of that plane sit in a higher binade than the row index
     "odd_rows_even_slices": lambda: Geometry(1000., 1500., np.array([0.1, 0.9, 2.3, 4.4]), 24, 401, 2.5, 0.05, 20, 20, 16, 2.0, 2.0, 2.0),
+    # angle lists closed under + 180 degrees (the march takes half-turn twins along): ragged and odd in-plane sizes, a detector
+    # wider than the volume's shadow (twins read the zero pads on the other side), detector offset in u (allowed: the half turn
+    # maps pixel u onto itself)
+    "twin_ragged": lambda: Geometry(1000., 1500., equispaced_angles(8) + 0.3, 50, 38, 1.3, 1.7, 40, 36, 20, 1.0, 1.25, 2.5),
+    "twin_odd_xy": lambda: Geometry(1000., 1500., equispaced_angles(10) + 0.05, 45, 30, 2.0, 2.0, 31, 29, 18, 2.0, 2.0, 2.0),
+    "twin_wide": lambda: Geometry(1000., 1500., equispaced_angles(6) + 0.2, 70, 44, 4.0, 6.0, 24, 24, 12, 2.0, 2.0, 2.0),
     "odd_rows_even_slices_coarse": lambda: Geometry(1000., 1500., equispaced_angles(5) + 0.05, 40, 33, 2.0, 2.0, 24, 24, 12, 2.0, 2.0, 2.0),
 }
 
@@ -122,6 +128,8 @@ def test_tma_staged_projector_equals_the_cached_march(cuda_lib, dev, name):
     g = GEOMS[name]()
     vol = f32(smooth_phantom(g, 3) if name != "c1" else make_config("c1").volume())
     G0, G1 = cb.Geometry.from_synth(g), cb.Geometry.from_synth(g)
+    G0.set_mirror_symmetry(False)                  # the plain march (the symmetric marches use one ray's table entries for its images)
+    G1.set_mirror_symmetry(False)
     G1.set_projector_staging(True)
     q0, q1 = torch.empty(G0.proj_shape, device=dev), torch.empty(G0.proj_shape, device=dev)
     cb.forward(G0, to_dev(vol, dev), q0)
@@ -139,13 +147,14 @@ def test_tma_staged_projector_equals_the_cached_march(cuda_lib, dev, name):
 
 
 @pytest.mark.parametrize("name", ["c1", "aniso_ragged", "wide_detector_misses", "short_arc_200deg", "fine_rows_multicross", "fine_columns",
-                                  "coarse_detector", "one_column", "odd_rows_even_slices", "odd_rows_even_slices_coarse"])
+                                  "coarse_detector", "one_column", "odd_rows_even_slices", "odd_rows_even_slices_coarse",
+                                  "twin_ragged", "twin_odd_xy", "twin_wide"])
 def test_plain_kernels_equal_the_mirrored_kernels(cuda_lib, dev, name):
     """Scans that are their own mirror image about z = 0 (nz even, detector centred in v) are marched two rays and gathered
-    two voxel rows at a time (cbct_set_mirror_symmetry, the default); the plain kernels (forced here, and the only ones for
-    odd nz or shifted panels) must give the same matrix: the march bit for bit (same arithmetic per ray), the gather within
-    the operator tolerance of the oracle and equal to the plain one to fp32 summation order, on phantom-like projections and
-    on Gaussian ones."""
+    two voxel rows at a time, and on angle lists closed under + 180 degrees the march also takes a ray's half-turn twin along
+    (cbct_set_mirror_symmetry, the default); the plain kernels (forced here, and the only ones for odd nz or shifted panels)
+    must give the same matrix: within the operator tolerance of the oracle and equal to each other to fp32 rounding, on
+    phantom-like inputs and on Gaussian ones."""
     import torch
     cb = cuda_lib
     g = GEOMS[name]()
@@ -156,7 +165,10 @@ def test_plain_kernels_equal_the_mirrored_kernels(cuda_lib, dev, name):
     q_p = run_forward(cb, G, vol, dev)
     G.set_mirror_symmetry(True)
     q_m = run_forward(cb, G, vol, dev)
-    assert np.array_equal(q_p, q_m)
+    # the z-mirrored march repeats the plain arithmetic per ray (bit-identical); where the angle list is closed under + 180
+    # degrees the march also takes the rays of angle a + 180 from the table entries of angle a (an equally good fp32 rounding
+    # of the same ray): equal to a few 1e-7
+    assert rel(q_m, q_p.astype(np.float64)) <= 0.5 * TOL_OP
     assert rel(q_m, o.forward(g, vol.astype(np.float64))) <= TOL_OP
     for y, tol in ((q_m, TOL_OP), (f32(gaussian_field(g.proj_shape, 21)), 5e-5)):
         ref = o.backproject(g, y.astype(np.float64))
@@ -173,7 +185,8 @@ def test_plain_kernels_equal_the_mirrored_kernels(cuda_lib, dev, name):
         G.set_mirror_symmetry(sym)
         d[sym] = torch.empty(G.vol_shape, device=dev)
         cb.data_gradient(G, to_dev(vol, dev), Y, d[sym])
-    assert rel(d[True].cpu().numpy(), d[False].cpu().numpy().astype(np.float64)) <= 2e-6
+    # (the residual P f - Y is a tenth of P f here, so a 1e-6 difference of the marches is a 1e-5 difference of the gradient)
+    assert rel(d[True].cpu().numpy(), d[False].cpu().numpy().astype(np.float64)) <= 2e-5
     G.close()
 
 
@@ -673,7 +686,7 @@ def test_sharded_halves_and_driver(cuda_lib, dev):
 
 
 @pytest.mark.parametrize("name", ["c1", "aniso_ragged", "odd_dims_axis_angles", "wide_detector_misses", "fine_rows_multicross", "coarse_detector",
-                                  "one_slice_one_row", "one_column", "odd_rows_even_slices_coarse"])
+                                  "one_slice_one_row", "one_column", "odd_rows_even_slices_coarse", "twin_ragged", "twin_odd_xy", "twin_wide"])
 def test_no_kernel_writes_outside_its_buffers(cuda_lib, dev, name):
     """compute-sanitizer is closed on this pool, so the library brings its own check: in guard mode every device buffer a handle
     owns (tables, padded copies, prefix sums, per-class gather outputs, ping-pong volumes, coarse-level data, FDK / V-cycle
