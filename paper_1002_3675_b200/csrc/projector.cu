@@ -230,16 +230,21 @@ forward_kernel(const DevGeom d, const int cls, const int2 *__restrict__ tiles, c
     }
 }
 
+bool march_is_mirrored(const cbct_geometry *g);
+
 // a2 alone: turns a plain projection q = P f (mode 0 of the march) into the residual the march's mode 1 / mode 2 would have
 // stored, with the very same operations (val = len * acc was stored; here len * (val - Y) or val - Y), so the result is bit
 // for bit the fused one.  Used by the host-buffer path, whose first projection starts before Y has arrived on the device.
-__global__ void __launch_bounds__(256) residual_kernel(const DevGeom d, float *__restrict__ q, const float *__restrict__ Y, const int mode)
+__global__ void __launch_bounds__(256) residual_kernel(const DevGeom d, float *__restrict__ q, const float *__restrict__ Y, const int mode,
+                                                       const int twin)
 {
     const int u = blockIdx.x * blockDim.x + threadIdx.x, v = blockIdx.y, a = blockIdx.z;
     if (u >= d.nu) return;
     const size_t o = ((size_t)a * d.nv + v) * d.nu + u;
     float val = q[o];
-    if (mode == 1) val = __fmul_rn(chord_scale(load_ray(d, a, u), __ldg(d.dz_mm + v)), __fsub_rn(val, __ldg(Y + o)));
+    // (the twin march takes the chord length of a second-half ray from its first-half twin's table entry; so does this)
+    const int at = twin && a >= d.na / 2 ? a - d.na / 2 : a;
+    if (mode == 1) val = __fmul_rn(chord_scale(load_ray(d, at, u), __ldg(d.dz_mm + v)), __fsub_rn(val, __ldg(Y + o)));
     else val = __fsub_rn(val, __ldg(Y + o));
     q[o] = val;
 }
@@ -248,7 +253,7 @@ cbct_status op_residual(cbct_geometry *g, float *d_q, const float *d_Y, int mode
 {
     ProfileScope ps(1, st);
     dim3 grid((g->nu + 255) / 256, g->nv, g->na);
-    residual_kernel<<<grid, 256, 0, st>>>(g->dev, d_q, d_Y, mode);
+    residual_kernel<<<grid, 256, 0, st>>>(g->dev, d_q, d_Y, mode, !g->fw_staged && march_is_mirrored(g) && g->twin_ok);
     CBCT_LAUNCH_CHECK();
     return CBCT_OK;
 }

@@ -362,9 +362,10 @@ def test_fbs_degenerate_cases(cuda_lib, dev):
     G.close()
 
 
-def test_host_entry_points(cuda_lib, dev):
+@pytest.mark.parametrize("name", ["aniso_ragged", "twin_ragged"])
+def test_host_entry_points(cuda_lib, dev, name):
     cb = cuda_lib
-    g = GEOMS["aniso_ragged"]()
+    g = GEOMS[name]()
     G = cb.Geometry.from_synth(g)
     vol = f32(smooth_phantom(g, 3))
     q = np.empty(g.proj_shape, dtype=np.float32)
