@@ -131,6 +131,73 @@ __global__ void __launch_bounds__(128) prefix_kernel(const DevGeom d, const floa
 }
 
 
+// The same prefix sums with the column cut into SEG segments of detector rows, one thread per (column, segment): a column
+// scanned by one thread leaves the GPU at 160 CTAs of 128 threads (c2) waiting on its own loads.  Pass 1 sums every segment
+// (compensated), the segment totals meet in shared memory, pass 2 rescans the segment (its rows now come from L1 / L2) on top
+// of the two-float total of the segments before it.  C(v).x + C(v).y is the sum of the rows below v to ~2^-48 as before; only
+// the rounding of the .x parts differs from the one-thread scan.
+template <int SEG>
+__global__ void __launch_bounds__(32 * SEG) prefix_seg_kernel(const DevGeom d, const float *__restrict__ in, const int scale,
+                                                              float *__restrict__ rs_out, float2 *__restrict__ C)
+{
+    __shared__ float2 tot[SEG][32];
+    const int lane = threadIdx.x, seg = threadIdx.y;
+    const int u = blockIdx.x * 32 + lane, a = blockIdx.y;
+    const bool in_range = u < d.nu;
+    const int len = (d.nv + SEG - 1) / SEG, v_lo = min(seg * len, d.nv), v_hi = min(v_lo + len, d.nv);
+    const int uc = min(u, d.nu - 1);
+    const RayXY r = load_ray(d, a, uc);
+    const float *p = in + (size_t)a * d.nv * d.nu + uc;
+    constexpr int PF = 8;
+    auto value = [&](float y, int v) { return scale ? y * chord_scale(r, __ldg(d.dz_mm + v)) : y; };
+    // pass 1: compensated sum of the segment
+    float s = 0.f, e = 0.f;
+    for (int v0 = v_lo; v0 < v_hi; v0 += PF) {
+        float y[PF];
+#pragma unroll
+        for (int q = 0; q < PF; ++q) y[q] = (v0 + q < v_hi) ? __ldg(p + (size_t)(v0 + q) * d.nu) : 0.f;
+#pragma unroll
+        for (int q = 0; q < PF; ++q) {
+            if (v0 + q >= v_hi) break;
+            const float yy = value(y[q], v0 + q);
+            const float t = __fadd_rn(s, yy);
+            e += two_sum_err(s, yy, t);
+            s = t;
+        }
+    }
+    tot[seg][lane] = make_float2(s, e);
+    __syncthreads();
+    // two-float total of the segments below this one
+    float os = 0.f, oe = 0.f;
+    for (int g = 0; g < seg; ++g) {
+        const float2 t2 = tot[g][lane];
+        const float t = __fadd_rn(os, t2.x);
+        oe += two_sum_err(os, t2.x, t) + t2.y;
+        os = t;
+    }
+    if (!in_range) return;
+    float *po = rs_out ? rs_out + (size_t)a * d.nv * d.nu + u : nullptr;
+    float2 *c = C + (size_t)a * (d.nv + 1) * d.nu + u;
+    if (seg == 0) *c = make_float2(0.f, 0.f);
+    // pass 2: the running sum of the segment on top of the offset
+    s = os; e = oe;
+    for (int v0 = v_lo; v0 < v_hi; v0 += PF) {
+        float y[PF];
+#pragma unroll
+        for (int q = 0; q < PF; ++q) y[q] = (v0 + q < v_hi) ? __ldg(p + (size_t)(v0 + q) * d.nu) : 0.f;
+#pragma unroll
+        for (int q = 0; q < PF; ++q) {
+            if (v0 + q >= v_hi) break;
+            const float yy = value(y[q], v0 + q);
+            if (scale && po) po[(size_t)(v0 + q) * d.nu] = yy;
+            const float t = __fadd_rn(s, yy);
+            e += two_sum_err(s, yy, t);
+            s = t;
+            c[(size_t)(v0 + q + 1) * d.nu] = make_float2(s, e);
+        }
+    }
+}
+
 #ifndef CBCT_BP_MINB
 #define CBCT_BP_MINB 8          // resident CTAs per SM the plain gather is compiled for (64 registers)
 #endif
@@ -359,6 +426,17 @@ cbct_status op_backproject_prefix(cbct_geometry *g, const float *d_in, int scale
     // kFixed: the column scales 1/s(a,u) sit behind the (half-size) integer prefix values in the same buffer
     PrefixT *Cp = reinterpret_cast<PrefixT *>(g->proj_prefix);
     float *inv_s = kFixed ? reinterpret_cast<float *>(Cp + (size_t)g->na * (g->nv + 1) * g->nu) : nullptr;
+#ifndef CBCT_BP_PREFIX_SEG
+#define CBCT_BP_PREFIX_SEG 8
+#endif
+    if constexpr (!kFixed && CBCT_BP_PREFIX_SEG > 1) {
+        if (g->nv >= 8 * CBCT_BP_PREFIX_SEG) {
+            dim3 sgrid((g->nu + 31) / 32, g->na), sblock(32, CBCT_BP_PREFIX_SEG);
+            prefix_seg_kernel<CBCT_BP_PREFIX_SEG><<<sgrid, sblock, 0, st>>>(g->dev, d_in, scale, d_rs_out, reinterpret_cast<float2 *>(g->proj_prefix));
+            CBCT_LAUNCH_CHECK();
+            return CBCT_OK;
+        }
+    }
     prefix_kernel<<<grid, 128, 0, st>>>(g->dev, d_in, scale, d_rs_out, Cp, inv_s, g->bp_run_max);
     CBCT_LAUNCH_CHECK();
     return CBCT_OK;

@@ -26,14 +26,28 @@ prolong_kernel(const float *__restrict__ c, float *__restrict__ f, int nx, int n
         float wj, wk;
         lin_pair(j, cy, ay, j0, j1, wj);
         lin_pair(k, cz, az, k0, k1, wk);
-        for (int i = threadIdx.x; i < nx; i += blockDim.x) {
-            int i0, i1;
-            float wi;
-            lin_pair(i, cx, ax, i0, i1, wi);
-            auto at = [&](int kk, int jj, int ii) { return __ldg(c + ((size_t)kk * cy + jj) * cx + ii); };
-            auto lx = [&](int kk, int jj) { return fmaf(wi, at(kk, jj, i1), (1.f - wi) * at(kk, jj, i0)); };
-            auto ly = [&](int kk) { return fmaf(wj, lx(kk, j1), (1.f - wj) * lx(kk, j0)); };
-            f[((size_t)k * ny + j) * nx + i] = fmaf(wk, ly(k1), (1.f - wk) * ly(k0));
+        auto at = [&](int kk, int jj, int ii) { return __ldg(c + ((size_t)kk * cy + jj) * cx + ii); };
+        // the (j, k) part of the interpolation of coarse column ii
+        auto col = [&](int ii) {
+            const float a0 = fmaf(wj, at(k0, j1, ii), (1.f - wj) * at(k0, j0, ii));
+            const float a1 = fmaf(wj, at(k1, j1, ii), (1.f - wj) * at(k1, j0, ii));
+            return fmaf(wk, a1, (1.f - wk) * a0);
+        };
+        float *frow = f + ((size_t)k * ny + j) * nx;
+        if (ax && (nx & 1) == 0 && (reinterpret_cast<unsigned long long>(f) & 7ull) == 0) {
+            // x coarsened: a thread makes the fine pair (2I, 2I+1) from the coarse columns I-1, I, I+1 (12 loads for two voxels
+            // instead of 16) and stores it as one float2
+            for (int I = threadIdx.x; I < cx; I += blockDim.x) {
+                const float cm = col(max(I - 1, 0)), c0 = col(I), cp = col(min(I + 1, cx - 1));
+                *reinterpret_cast<float2 *>(frow + 2 * I) = make_float2(fmaf(0.25f, cm, 0.75f * c0), fmaf(0.25f, cp, 0.75f * c0));
+            }
+        } else {
+            for (int i = threadIdx.x; i < nx; i += blockDim.x) {
+                int i0, i1;
+                float wi;
+                lin_pair(i, cx, ax, i0, i1, wi);
+                frow[i] = fmaf(wi, col(i1), (1.f - wi) * col(i0));
+            }
         }
     }
 }
