@@ -126,12 +126,15 @@ cbct_status cbct_set_projector_staging(cbct_geometry *g, int on);
 cbct_status cbct_backproject(const cbct_geometry *g, const float *d_proj, float *d_vol, void *cuda_stream);
 
 /*
- * Whether the projector and the exact backprojector may use the scan's mirror symmetry about the central plane z = 0: on = 1
- * (the default) lets a thread march ray (u, v) together with its mirror image (u, nv-1-v), and gather a voxel row k together
- * with its mirror image nz-1-k, from one evaluation of the z arithmetic, wherever the geometry is its own mirror image (nz
- * even, no detector shift in v; the projector also needs nv even); on = 0 forces the plain kernels.  Same matrix entries
- * either way (the mirrored ray has the mirrored chords, O1); results equal to fp32 rounding.  Applies to this handle and its
- * coarse levels.
+ * Whether the projector and the exact backprojector may use the symmetries of the scan: on = 1 (the default) lets a thread
+ *   - march ray (u, v) together with its mirror image (u, nv-1-v) about the central plane z = 0, and gather a voxel row k together
+ *     with its mirror image nz-1-k, from one evaluation of the z arithmetic, wherever the geometry is its own mirror image (nz
+ *     even, no detector shift in v; the projector also needs nv even);
+ *   - march, in addition, the half-turn twins of those rays (angle a + n_angles/2, same pixel, voxels point-reflected about the
+ *     rotation axis) from the same ray arithmetic, wherever angles[a + n_angles/2] = angles[a] + pi for every a < n_angles/2
+ *     (the second-half rays are then marched from their twin's table entries: an equally good fp32 rounding of the same ray);
+ * on = 0 forces the plain kernels.  Same matrix entries either way (O1); results equal to fp32 rounding.  Applies to this
+ * handle and its coarse levels.
  */
 cbct_status cbct_set_mirror_symmetry(cbct_geometry *g, int on);
 
