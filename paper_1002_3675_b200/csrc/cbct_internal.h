@@ -79,6 +79,7 @@ struct cbct_geometry {
     int2 *d_tiles[2] = {nullptr, nullptr};   // forward work list per class: (angle, u0)
     int n_tiles[2] = {0, 0};
     int n_tiles_half[2] = {0, 0};             // tiles of the first half turn (angle index < na/2): the twin march launches only these
+    int last_march_twin = 0;                  // the last projection on this handle was made by the twin march (op_residual follows it)
     bool twin_ok = false;                     // angle a + na/2 = angle a + 180 degrees for every a < na/2 (and mirror symmetry switched on)
     unsigned char *d_angle_has[2] = {nullptr, nullptr};   // [na] does this angle have rays of the class
     std::vector<unsigned char> h_angle_has[2];

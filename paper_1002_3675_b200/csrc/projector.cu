@@ -253,7 +253,7 @@ cbct_status op_residual(cbct_geometry *g, float *d_q, const float *d_Y, int mode
 {
     ProfileScope ps(1, st);
     dim3 grid((g->nu + 255) / 256, g->nv, g->na);
-    residual_kernel<<<grid, 256, 0, st>>>(g->dev, d_q, d_Y, mode, !g->fw_staged && march_is_mirrored(g) && g->twin_ok);
+    residual_kernel<<<grid, 256, 0, st>>>(g->dev, d_q, d_Y, mode, g->last_march_twin);
     CBCT_LAUNCH_CHECK();
     return CBCT_OK;
 }
@@ -278,6 +278,7 @@ cbct_status op_forward_padded(cbct_geometry *g, float *d_out, const float *d_Y, 
 #define CBCT_FW_VT 2
 #endif
     constexpr int V = CBCT_FW_V, WARPS = CBCT_FW_WARPS;
+    g->last_march_twin = 0;
     if (g->fw_staged) {
         int done = 0;
         CBCT_TRY(op_forward_padded_tma(g, d_out, d_Y, mode, st, &done));
@@ -287,6 +288,7 @@ cbct_status op_forward_padded(cbct_geometry *g, float *d_out, const float *d_Y, 
     // every ray belongs to a tile of its class (geometry.cu), so every output element is written: 0 / -Y / -l Y for a
     // ray that misses the volume
     const bool mirror = march_is_mirrored(g);
+    g->last_march_twin = mirror && g->twin_ok;           // op_residual follows the march that made the projection
     for (int c = 0; c < 2; ++c) {
         if (g->n_tiles[c] == 0) continue;
         if (mirror && g->twin_ok) {
