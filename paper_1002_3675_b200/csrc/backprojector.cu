@@ -57,6 +57,9 @@ __device__ __forceinline__ float two_sum_err(float a, float b, float s)
 #ifndef CBCT_BP_FIXED
 #define CBCT_BP_FIXED 0
 #endif
+#ifndef CBCT_BP_PACKED
+#define CBCT_BP_PACKED 1
+#endif
 // Prefix sums along v in one of two forms.  kFixed = false: (sum, two-sum compensation) float pairs.  kFixed = true: 32-bit
 // fixed point with wrap-around: every column (a, u) is scaled by a power of two s(a,u) such that any run of at most
 // `run_max` detector rows sums to less than 2^30 in magnitude, rounded to integers and summed modulo 2^32, so the difference
@@ -227,12 +230,22 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
     if (i >= cg.nmaj) return;                          // warp-uniform
     const bool valid = j < cg.nmin;
 
-    float acc[KC], accL[MIRROR ? KC : 1];
+    // kPacked (MIRROR, float prefix sums): a voxel row and its mirror image accumulate as the two halves of one float2, updated
+    // by sm_100's packed fp32 instructions (FFMA2: two fused multiply-adds, one issue slot) — the kernel is bound by issue slots
+    constexpr bool kPacked = MIRROR && !kFixed && CBCT_BP_PACKED != 0;
+    float2 accP[kPacked ? KC : 1];
+    if constexpr (kPacked) {
 #pragma unroll
-    for (int q = 0; q < KC; ++q) acc[q] = 0.f;
-    if constexpr (MIRROR) {
+        for (int q = 0; q < KC; ++q) accP[q] = make_float2(0.f, 0.f);
+    }
+    float acc[kPacked ? 1 : KC], accL[MIRROR && !kPacked ? KC : 1];
+    if constexpr (!kPacked) {
 #pragma unroll
-        for (int q = 0; q < KC; ++q) accL[q] = 0.f;
+        for (int q = 0; q < KC; ++q) acc[q] = 0.f;
+        if constexpr (MIRROR) {
+#pragma unroll
+            for (int q = 0; q < KC; ++q) accL[q] = 0.f;
+        }
     }
 
     // the column's x-y square in mm (candidate search only; the accept test is exact)
@@ -338,7 +351,11 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
                     // ray lying in it — odd nv, even nz — crosses nothing and belongs to the row above; the mirrored gather meets that
                     // plane only as q = 0 of the chunk with zk0 = 0, where xT0 = xTn0 = cv)
                     int vT, vTn;
-                    if constexpr (MIRROR) {
+                    if constexpr (kPacked) {                   // both bounds by one packed FMA
+                        const float2 xb = __ffma2_rn(make_float2((float)q, (float)q), make_float2(cT, cTn), make_float2(xT0, xTn0));
+                        vT = (int)ceilf(xb.x);
+                        vTn = (int)ceilf(xb.y);
+                    } else if constexpr (MIRROR) {
                         vT = (int)ceilf(fmaf((float)q, cT, xT0));
                         vTn = (int)ceilf(fmaf((float)q, cTn, xTn0));
                     } else {
@@ -373,9 +390,9 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
                     // in it belongs to the row above it on both sides), crossing ray nv-1-vs, rising <-> falling
                     [[maybe_unused]] PrefixT c2L;
                     [[maybe_unused]] float dn = 0.f;                    // moved DOWN across the mirrored plane
+                    [[maybe_unused]] float yL = 0.f;
                     if constexpr (MIRROR) {
                         c2L = (q == 0 && zk0 == 0.f) ? c2 : __ldg(reinterpret_cast<const PrefixT *>(row_ptr(CuT, vT, npitchC)));
-                        float yL = 0.f;
                         if (dlt != 0) yL = __ldg(reinterpret_cast<const float *>(row_ptr(RuT, vs, npitchR)));
                         dn = fs * yL;
                     }
@@ -388,15 +405,37 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
                             if constexpr (MIRROR) dn = fmaf(f2, __ldg(reinterpret_cast<const float *>(row_ptr(RuT, v, npitchR))), dn);
                         }
                     }
-                    if (q > 0) {
-                        acc[q > 0 ? q - 1 : 0] = fmaf(wr, run_sum(c2, c1), acc[q > 0 ? q - 1 : 0]) - up;
-                        if constexpr (MIRROR) {
-                            accL[q > 0 ? q - 1 : 0] = fmaf(wr, run_sum(c1L, c2L), accL[q > 0 ? q - 1 : 0]) - dn;
+                    if constexpr (kPacked && !MULTI) {
+                        // (upper row, mirrored row) side by side: c2 - c1 and c1L - c2L as packed FMAs with -1, the run sums, then
+                        // three packed FMAs move w run - up into row q-1 and up into row q on both sides
+                        const float2 m1 = make_float2(-1.f, -1.f), yy = make_float2(yq, yL);
+                        if (q > 0) {
+                            const float2 dU = __ffma2_rn(c1, m1, c2), dL = __ffma2_rn(c2L, m1, c1L);
+                            const float2 run = make_float2(dU.x + dU.y, dL.x + dL.y);
+                            accP[q > 0 ? q - 1 : 0] = __ffma2_rn(make_float2(wr, wr), run, accP[q > 0 ? q - 1 : 0]);
+                            accP[q > 0 ? q - 1 : 0] = __ffma2_rn(make_float2(-fs, -fs), yy, accP[q > 0 ? q - 1 : 0]);
                         }
-                    }
-                    if (q < KC) {
-                        acc[q < KC ? q : 0] += up;
-                        if constexpr (MIRROR) accL[q < KC ? q : 0] += dn;
+                        if (q < KC) accP[q < KC ? q : 0] = __ffma2_rn(make_float2(fs, fs), yy, accP[q < KC ? q : 0]);
+                    } else if constexpr (kPacked) {           // the rare several-crossings loop: the same rows, one half at a time
+                        if (q > 0) {
+                            accP[q > 0 ? q - 1 : 0].x = fmaf(wr, run_sum(c2, c1), accP[q > 0 ? q - 1 : 0].x) - up;
+                            accP[q > 0 ? q - 1 : 0].y = fmaf(wr, run_sum(c1L, c2L), accP[q > 0 ? q - 1 : 0].y) - dn;
+                        }
+                        if (q < KC) {
+                            accP[q < KC ? q : 0].x += up;
+                            accP[q < KC ? q : 0].y += dn;
+                        }
+                    } else {
+                        if (q > 0) {
+                            acc[q > 0 ? q - 1 : 0] = fmaf(wr, run_sum(c2, c1), acc[q > 0 ? q - 1 : 0]) - up;
+                            if constexpr (MIRROR) {
+                                accL[q > 0 ? q - 1 : 0] = fmaf(wr, run_sum(c1L, c2L), accL[q > 0 ? q - 1 : 0]) - dn;
+                            }
+                        }
+                        if (q < KC) {
+                            acc[q < KC ? q : 0] += up;
+                            if constexpr (MIRROR) accL[q < KC ? q : 0] += dn;
+                        }
                     }
                     c1 = c2;
                     if constexpr (MIRROR) c1L = c2L;
@@ -412,8 +451,8 @@ backproject_kernel(const DevGeom d, const int cls, const unsigned char *__restri
     for (int q = 0; q < KC; ++q) {
         const int k = k0 + q;
         if (k < d.nz) {
-            G[((size_t)k * cg.nmaj + i) * cg.nmin + j] = acc[q];
-            if constexpr (MIRROR) G[((size_t)(d.nz - 1 - k) * cg.nmaj + i) * cg.nmin + j] = accL[q];
+            G[((size_t)k * cg.nmaj + i) * cg.nmin + j] = kPacked ? accP[kPacked ? q : 0].x : acc[kPacked ? 0 : q];
+            if constexpr (MIRROR) G[((size_t)(d.nz - 1 - k) * cg.nmaj + i) * cg.nmin + j] = kPacked ? accP[kPacked ? q : 0].y : accL[kPacked ? 0 : q];
         }
     }
 }
