@@ -192,6 +192,32 @@ cbct_status cbct_energy(const cbct_geometry *g, const float *d_f, const float *d
                         float mu, float eps, double *h_out3, void *cuda_stream);
 
 /*
+ * The TV term of that energy for callers that must not allocate device memory (O3):
+ *   *d_out = TV_eps(f) = sum over voxels of sqrt(dx^2 + dy^2 + dz^2 + eps^2)      (E1_eps of cbct_energy = *d_out / N_vox)
+ * with the same differences, fp32 terms and fp64 accumulation as cbct_energy; the two agree to the rounding of the fp64 sums.
+ * Who this is for: cbct_energy keeps its per-block partial sums in scratch that the handle obtains with cudaMalloc, and a handle
+ * cannot even be created without cudaMalloc.  A host application that has given the whole card to its own memory pool, a monitor
+ * running beside a reconstruction that fills HBM on purpose, or a loop that cannot afford the device-wide stall of an
+ * allocation cannot use either.  This call needs no handle and allocates nothing, on the device or on the host (no cudaMalloc,
+ * cudaFree, events or library routine that allocates): the partial sums go to a fixed 128 KiB array that is part of the
+ * library image (every GPU on which the library is loaded carries it until the process exits, used or not).
+ *   d_f                 DEVICE, nz*ny*nx floats (x fastest), read only
+ *   nx..nz, hx..hz      volume dims and voxel size in mm; no geometry handle is involved
+ *   d_out               DEVICE, one double, overwritten; caller-owned like d_f
+ * Limit: nx*ny*nz <= 134 217 728 (= 512^3, the largest volume in BASELINE.json) and each dim <= 16384; larger volumes return
+ * CBCT_ERR_SHAPE with a message and launch nothing.  INVALID_ARG for NULL pointers, non-positive dims or spacings, eps < 0.
+ * Asynchronous on cuda_stream; nothing is synchronised.
+ * First call on a device: with that device current, the call looks up the device address of the array once
+ * (cudaGetSymbolAddress) and remembers it per device ordinal; make this first call before any stream capture begins.
+ * Sharing: there is ONE array per GPU, used by every call from every thread and stream, and it keeps the previous call's
+ * partial sums.  No part of it has to start at zero (each call writes every slot it later reads), but two calls that overlap
+ * on the GPU - issued on different streams, from one host thread or several - race on it and may both return garbage.  Order
+ * such calls on one stream or with events.  (Separate processes have separate copies of the array.)
+ */
+cbct_status cbct_tv_value_noalloc(const float *d_f, int nx, int ny, int nz, double hx_mm, double hy_mm, double hz_mm,
+                                  float eps, double *d_out, void *cuda_stream);
+
+/*
  * The hot path: Algorithm A1 inside a coarse-to-fine cascade (O5/O6).
  * For level l = n_levels-1 (coarsest) ... 0 (finest = g), n_outer_per_level[] listed COARSEST FIRST:
  *   repeat n_outer times:

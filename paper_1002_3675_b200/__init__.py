@@ -11,5 +11,5 @@ from .binding import (  # noqa: F401
     forward, backproject, backproject_eq2, set_backprojector, BACKPROJECTOR_EXACT, BACKPROJECTOR_EQ2, tv_prox, fbs_reconstruct, fbs_reconstruct_until, data_gradient, prox_step, energy, prolong, restrict, bin2x2,
     profile_enable, profile_read, PROFILE_TAGS, set_guard_mode,
     forward_host, backproject_host, tv_prox_host, fbs_reconstruct_host,
-    fbs_vcycle, fdk_reconstruct, fbs_reconstruct_sharded, CascadeOps, ALLREDUCE_FN,
+    fbs_vcycle, fdk_reconstruct, tv_value_noalloc, fbs_reconstruct_sharded, CascadeOps, ALLREDUCE_FN,
 )

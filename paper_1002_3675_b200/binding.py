@@ -18,7 +18,7 @@ SYMBOLS = (
     "cbct_fbs_reconstruct_sharded", "cbct_cascade_run", "cbct_set_projector_staging", "cbct_set_mirror_symmetry", "cbct_set_guard_mode", "cbct_check_guards", "cbct_geometry_destroy", "cbct_geometry_query", "cbct_geometry_coarsen",
     "cbct_forward", "cbct_backproject", "cbct_backproject_eq2", "cbct_set_backprojector", "cbct_tv_prox", "cbct_prolong", "cbct_restrict", "cbct_bin2x2",
     "cbct_energy", "cbct_data_gradient", "cbct_prox_step", "cbct_fbs_reconstruct", "cbct_fbs_reconstruct_until", "cbct_forward_host", "cbct_backproject_host", "cbct_tv_prox_host",
-    "cbct_fbs_reconstruct_host", "cbct_profile_enable", "cbct_profile_read", "cbct_launch_count", "cbct_device_bytes", "cbct_last_error",
+    "cbct_fbs_reconstruct_host", "cbct_tv_value_noalloc", "cbct_profile_enable", "cbct_profile_read", "cbct_launch_count", "cbct_device_bytes", "cbct_last_error",
 )
 
 
@@ -95,6 +95,7 @@ def load():
     L.cbct_backproject_host.argtypes = [vp, fp, fp, vp]
     L.cbct_tv_prox_host.argtypes = [vp, fp, fp, f, f, f, i, vp]
     L.cbct_fbs_reconstruct_host.argtypes = [vp, fp, fp, i, ip, i, f, f, f, f, fp, dp, vp]
+    L.cbct_tv_value_noalloc.argtypes = [fp, i, i, i, d, d, d, f, vp, vp]
     L.cbct_profile_enable.argtypes = [i]
     L.cbct_profile_read.argtypes = [dp, C.POINTER(C.c_ulonglong), i]
     L.cbct_launch_count.restype = C.c_ulonglong
@@ -302,6 +303,22 @@ def energy(g: Geometry, d_f, d_Y, mu, eps, stream=None):
     out = (C.c_double * 3)()
     _check(load().cbct_energy(g._h, _dev(d_f, g.n_vox, "d_f"), _dev(d_Y, g.n_proj, "d_Y"), float(mu), float(eps), out, _stream(stream)))
     return {"E_eps": out[0], "E1_eps": out[1], "E2": out[2]}
+
+
+def tv_value_noalloc(d_f, hx, hy, hz, eps, d_out, stream=None):
+    """cbct_tv_value_noalloc: d_out[0] = TV_eps(d_f) for callers that may not allocate device memory (an application whose
+    own pool owns the whole card, a monitor beside a reconstruction that fills HBM, a loop that cannot take an allocation's
+    device-wide stall).  d_f: contiguous float32 CUDA tensor of shape (nz, ny, nx), at most 512^3 voxels; d_out: CUDA
+    float64 tensor with one element, supplied by the caller.  No handle; the binding allocates nothing either.  All calls
+    on a GPU share one fixed scratch array: keep them ordered on one stream (or with events)."""
+    import torch
+    if not (isinstance(d_f, torch.Tensor) and d_f.is_cuda and d_f.dtype == torch.float32 and d_f.is_contiguous() and d_f.dim() == 3):
+        raise TypeError("d_f: expected a contiguous float32 CUDA tensor of shape (nz, ny, nx)")
+    if not (isinstance(d_out, torch.Tensor) and d_out.is_cuda and d_out.dtype == torch.float64 and d_out.numel() == 1):
+        raise TypeError("d_out: expected a float64 CUDA tensor with one element")
+    nz, ny, nx = (int(x) for x in d_f.shape)
+    _check(load().cbct_tv_value_noalloc(d_f.data_ptr(), nx, ny, nz, float(hx), float(hy), float(hz), float(eps),
+                                        d_out.data_ptr(), _stream(stream)))
 
 
 def _outer(n_levels: int, n_outer: Sequence[int]):
