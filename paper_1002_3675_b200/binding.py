@@ -358,7 +358,9 @@ def fdk_reconstruct(g: Geometry, d_Y, d_vol, stream=None):
 def fbs_reconstruct_sharded(g: Geometry, d_Y_local, d_f0, n_levels, n_outer, n_inner, step, mu, eps, omega, n_angles_total,
                             allreduce, d_G_scratch, d_f_out, stream=None):
     """cbct_fbs_reconstruct_sharded.  `allreduce(count)` must sum the first `count` floats of d_G_scratch over the ranks in
-    place (None = single rank).  Argument marshalling only: the cascade and its constants live behind the C ABI."""
+    place (None = single rank); it is called with the library's stream as torch's current stream, so torch.distributed
+    collectives and plain torch ops inside it are ordered with the kernels around them whatever `stream` is.
+    Argument marshalling only: the cascade and its constants live behind the C ABI."""
     arr, _ = _outer(n_levels, n_outer)
     gptr = _dev(d_G_scratch, g.n_vox, "d_G_scratch")
     err = []
@@ -367,7 +369,13 @@ def fbs_reconstruct_sharded(g: Geometry, d_Y_local, d_f0, n_levels, n_outer, n_i
         try:
             if int(d_buf) != gptr:
                 raise RuntimeError("all-reduce called on a buffer that is not d_G_scratch")
-            allreduce(int(count))
+            # cbct.h: the exchange must be ordered on the stream the library hands over.  torch orders its collectives (and
+            # any other torch op the callback runs) against torch's CURRENT stream, so that stream is made current here
+            # (NULL = the legacy default stream, which is torch's default stream).
+            import torch
+            s = torch.cuda.ExternalStream(int(st)) if st else torch.cuda.default_stream()
+            with torch.cuda.stream(s):
+                allreduce(int(count))
             return 0
         except Exception as e:            # never let an exception cross the C frame
             err.append(e)

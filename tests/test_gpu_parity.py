@@ -686,6 +686,52 @@ def test_sharded_halves_and_driver(cuda_lib, dev):
     G_all.close()
 
 
+def test_sharded_driver_exchange_is_ordered_on_a_side_stream(cuda_lib, dev):
+    """The exchange callback must run on the stream the library hands it, not on torch's current stream.  Stand-in for two
+    ranks that hold the same views: the "sum over ranks" doubles the gradient volume in place and n_angles_total doubles,
+    so c G is unchanged bit for bit (factors of two) and the result must equal cbct_fbs_reconstruct's.  The whole cascade
+    runs on a side stream while torch's current stream stays the default one: an exchange issued on the current stream would
+    be unordered against the kernels on either side of it."""
+    import torch
+    from paper_1002_3675_b200.sharded import fbs_reconstruct_sharded
+    cb = cuda_lib
+    cfg = make_config("c3", shrink=4)          # 128 x 128 x 16: kernels long enough for a misplaced exchange to overtake them
+    g = cfg.geom
+    G = cb.Geometry.from_synth(g)
+    d_Y = to_dev(f32(cfg.projections()), dev)
+    args = (cfg.n_inner, cfg.step, cfg.mu, cfg.eps, cfg.omega)
+    f_ref = torch.empty(G.vol_shape, device=dev)
+    cb.fbs_reconstruct(G, d_Y, None, 2, [4, 3], *args, f_ref)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    Gs = torch.empty(G.vol_shape, device=dev)
+    f_side = torch.empty(G.vol_shape, device=dev)
+    seen = []
+
+    def twice(count):
+        seen.append(torch.cuda.current_stream().cuda_stream)
+        Gs.view(-1)[:count].mul_(2.0)
+
+    cb.fbs_reconstruct_sharded(G, d_Y, None, 2, [4, 3], *args, 2 * g.n_angles, twice, Gs, f_side, stream=side)
+    side.synchronize()
+    assert seen == [side.cuda_stream] * 7
+    assert torch.equal(f_side, f_ref)
+
+    class OneRankDist:                         # the wiring of sharded.py with a one-rank stand-in for torch.distributed
+        class ReduceOp:
+            SUM = 0
+
+        @staticmethod
+        def all_reduce(t, op=None):
+            seen.append(torch.cuda.current_stream().cuda_stream)
+
+    del seen[:]
+    f_one = fbs_reconstruct_sharded(G, d_Y, None, 2, [4, 3], *args, g.n_angles, OneRankDist, stream=side)
+    side.synchronize()
+    assert seen == [side.cuda_stream] * 7 and torch.equal(f_one, f_ref)
+    G.close()
+
+
 @pytest.mark.parametrize("name", ["c1", "aniso_ragged", "odd_dims_axis_angles", "wide_detector_misses", "fine_rows_multicross", "coarse_detector",
                                   "one_slice_one_row", "one_column", "odd_rows_even_slices_coarse", "twin_ragged", "twin_odd_xy", "twin_wide"])
 def test_no_kernel_writes_outside_its_buffers(cuda_lib, dev, name):
