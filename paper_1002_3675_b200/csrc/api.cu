@@ -245,7 +245,11 @@ cbct_status op_fbs_level(cbct_geometry *g, const float *d_Y, float *f, int n_out
     // Small volumes are launch-bound (c1: a dozen kernels of 5-10 us per iteration): after one eager iteration (which makes
     // every allocation) the iteration is captured once into a CUDA graph on an internal stream and replayed on the caller's.
     // Any failure to capture falls back to eager launches.
-    cudaGraphExec_t gexec = nullptr;
+    struct GraphExecGuard {                                      // destroyed on every way out of this function, error returns included
+        cudaGraphExec_t e = nullptr;
+        ~GraphExecGuard() { if (e) cudaGraphExecDestroy(e); }
+    } guard;
+    cudaGraphExec_t &gexec = guard.e;
     const bool want_graph = !trace && rel_tol == 0.f && !y_gate && !cbct_profile_is_on() && n_outer >= 6 && g->n_vox() <= ((size_t)1 << 20);
     for (int it = 0; it < n_outer; ++it) {
         if (rel_tol > 0.f) CBCT_CUDA(cudaMemcpyAsync(g->vol_c, f, g->n_vox() * sizeof(float), cudaMemcpyDeviceToDevice, st));
@@ -284,7 +288,6 @@ cbct_status op_fbs_level(cbct_geometry *g, const float *d_Y, float *f, int n_out
             if (std::sqrt(g->h_red[0]) <= (double)rel_tol * std::sqrt(g->h_red[1])) break;
         }
     }
-    if (gexec) cudaGraphExecDestroy(gexec);
     return CBCT_OK;
 }
 

@@ -686,6 +686,37 @@ def test_sharded_halves_and_driver(cuda_lib, dev):
     G_all.close()
 
 
+def test_graph_replay_equals_eager_launches(cuda_lib, dev):
+    """Small volumes replay one captured outer iteration as a CUDA graph (n_outer >= 6, <= 2^20 voxels, no trace, no stopping
+    rule, profiling off); per-kernel profiling forces the same iterations to be launched eagerly.  Same kernels, same
+    arguments, same order: the volumes must be equal bit for bit, with either backprojector and with / without TV sweeps."""
+    import torch
+    cb = cuda_lib
+    cfg = make_config("c1")
+    g = cfg.geom
+    d_Y = to_dev(f32(cfg.projections()), dev)
+    for mode, n_inner, n_levels, n_outer in ((cb.BACKPROJECTOR_EXACT, cfg.n_inner, 1, [9]), (cb.BACKPROJECTOR_EXACT, 0, 1, [7]),
+                                             (cb.BACKPROJECTOR_EQ2, cfg.n_inner, 1, [8]), (cb.BACKPROJECTOR_EXACT, 2, 2, [6, 7])):
+        res = []
+        for eager in (False, True):
+            G = cb.Geometry.from_synth(g)                 # a fresh handle each time: the first iteration allocates in both runs
+            cb.set_backprojector(G, mode)
+            f = torch.empty(G.vol_shape, device=dev)
+            cb.profile_enable(eager)
+            try:
+                n0 = cb.launch_count()
+                cb.fbs_reconstruct(G, d_Y, None, n_levels, n_outer, n_inner, cfg.step, cfg.mu, cfg.eps, cfg.omega, f)
+                torch.cuda.synchronize()
+                res.append((f.clone(), cb.launch_count() - n0))
+            finally:
+                cb.profile_enable(False)
+                cb.profile_read(reset=True)
+            G.close()
+        assert torch.equal(res[0][0], res[1][0]), (mode, n_inner, n_levels)
+        assert res[0][1] == res[1][1]                      # the launch counter counts replayed kernels like launched ones
+        assert float(res[0][0].abs().sum()) > 0
+
+
 def test_sharded_driver_exchange_is_ordered_on_a_side_stream(cuda_lib, dev):
     """The exchange callback must run on the stream the library hands it, not on torch's current stream.  Stand-in for two
     ranks that hold the same views: the "sum over ranks" doubles the gradient volume in place and n_angles_total doubles,
