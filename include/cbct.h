@@ -80,7 +80,8 @@ cbct_status cbct_geometry_create_ex(double sad_mm, double sdd_mm,
                                     int nx, int ny, int nz, double hx_mm, double hy_mm, double hz_mm,
                                     cbct_geometry **out);
 
-/* Frees the handle, its coarse-level handles and all scratch.  NULL is allowed.  Synchronises the device. */
+/* Frees the handle, its coarse-level handles and all scratch.  NULL is allowed.  Synchronises the device.  Every pointer
+ * obtained from cbct_geometry_coarsen on this handle (or on its coarse levels) is dangling afterwards. */
 void cbct_geometry_destroy(cbct_geometry *g);
 
 /* Writes {n_angles, nu, nv, nx, ny, nz} to h_dims6 and {du, dv, hx, hy, hz} to h_sizes5 (either may be NULL). */
@@ -90,7 +91,8 @@ cbct_status cbct_geometry_query(const cbct_geometry *g, int *h_dims6, double *h_
  * Next-coarser multigrid level ("multi-grid method"; reading O6/Q11): every axis whose spacing
  * is <= sqrt(2) * min(hx,hy,hz) is coarsened by 2 (dims halve, spacing doubles); the detector is
  * binned 2x2 (pitch doubles) iff both x and y were coarsened.  The returned handle is OWNED BY `g`
- * (freed with it; repeated calls return the same handle).  h_flags4 (may be NULL) receives
+ * (freed with it, or earlier by a cbct_set_detector_binning call that changes the choice: do not keep the pointer across
+ * either; repeated calls return the same handle until then).  h_flags4 (may be NULL) receives
  * {x coarsened, y coarsened, z coarsened, detector binned}.
  * Errors: SHAPE for an odd dimension on an axis that must coarsen (or odd nu/nv when binning).
  */
@@ -100,6 +102,9 @@ cbct_status cbct_geometry_coarsen(const cbct_geometry *g, cbct_geometry **out_co
  * NEXT-3 (reading Q20): whether the coarse multigrid levels bin the detector 2x2 (on = 1, the default, O6) or keep the
  * detector and the data at full resolution (on = 0).  Changing the choice drops the handle's existing coarse levels
  * (synchronises the device); they are rebuilt on demand.  Applies to every cascade / V-cycle run on this handle.
+ * INVALIDATES every coarse-level pointer cbct_geometry_coarsen has returned for this handle and for its coarse levels (the
+ * whole chain is freed): using one afterwards is a use-after-free.  Call cbct_geometry_coarsen again to get the new level.
+ * A call that does not change the choice frees nothing.
  */
 cbct_status cbct_set_detector_binning(cbct_geometry *g, int on);
 
@@ -276,9 +281,14 @@ cbct_status cbct_fbs_vcycle(const cbct_geometry *g, const float *d_Y, const floa
  * NEXT-4. The FDK reconstruction the paper compares against (Feldkamp-Davis-Kress, ref. 1 at P:147; Fig. 1(d) P:105,
  * Fig. 2), reading Q22: d_vol = (pi/N_theta) sum_theta SAD^2/U^2 q_theta(u*,v*) with q the cosine-weighted
  * (SDD/sqrt(SDD^2+u^2+v^2)) projections filtered along u by the band-limited ramp kernel at pitch du SAD/SDD, U the distance
- * of the voxel from the source along the central ray, bilinear interpolation, zero outside the detector.  Valid for equally
- * spaced views over a full rotation (no short-scan or half-fan redundancy weights, no apodisation).  d_vol is overwritten.
- * Errors: SHAPE if nu > 17066 (the filter keeps a zero-padded row in shared memory).
+ * of the voxel from the source along the central ray, bilinear interpolation, zero outside the detector (detector positions
+ * in fp64, weights and sums in fp32).  Valid for equally spaced views over a full rotation only (no short-scan or half-fan
+ * redundancy weights, no apodisation): the angle list must be angles[0] +- 2 pi a / n_angles to 1e-6 of a step, in list order;
+ * any other list (a 200 degree arc, a list with a gap or a repeated view) is refused.  A panel shift (cbct_geometry_create_ex) is
+ * applied as such: right for a slightly miscentred panel that still sees the whole object, NOT for a half-fan scan, which
+ * needs the redundancy weights this routine does not have.  d_vol is overwritten.
+ * Errors: SHAPE if the views are not equally spaced over a full turn, or if nu > 8533 (the filter keeps a zero-padded fp64
+ * row in shared memory).
  */
 cbct_status cbct_fdk_reconstruct(const cbct_geometry *g, const float *d_Y, float *d_vol, void *cuda_stream);
 

@@ -3,6 +3,7 @@ from __future__ import annotations
 
 import ctypes as C
 import os
+import weakref
 from typing import Optional, Sequence
 
 import numpy as np
@@ -175,6 +176,7 @@ class Geometry:
     def __init__(self, sad, sdd, angles, nu, nv, du, dv, nx, ny, nz, hx, hy, hz, off_u=0.0, off_v=0.0, _handle=None, _parent=None):
         L = load()
         self._parent = _parent            # coarse handles are owned by their fine handle
+        self._children = []               # weak references to the coarse-level wrappers coarsen() has handed out
         if _handle is not None:
             self._h = _handle
         else:
@@ -223,7 +225,19 @@ class Geometry:
         h = C.c_void_p()
         fl = (C.c_int * 4)()
         _check(load().cbct_geometry_coarsen(self._h, C.byref(h), fl))
-        return Geometry(0, 0, None, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, _handle=h, _parent=self), tuple(bool(x) for x in fl)
+        c = Geometry(0, 0, None, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, _handle=h, _parent=self)
+        self._children = [r for r in self._children if r() is not None] + [weakref.ref(c)]
+        return c, tuple(bool(x) for x in fl)
+
+    def _drop_children(self):
+        """The library is about to free (or has freed) this handle's coarse levels: every wrapper that still points at one
+        loses its pointer, so that a later use is a clean CBCT_ERR_INVALID_ARG (NULL handle) instead of a use-after-free."""
+        for r in self._children:
+            c = r()
+            if c is not None:
+                c._drop_children()
+                c._h = None
+        self._children = []
 
     def set_projector_staging(self, on: bool):
         """Projector fed by TMA-staged shared-memory bricks (True) or by the L1-cached march (False, default)."""
@@ -240,7 +254,9 @@ class Geometry:
         return int(n.value)
 
     def set_detector_binning(self, on: bool):
-        """Coarse levels bin the detector 2x2 (default) or keep it at full resolution; drops existing coarse levels."""
+        """Coarse levels bin the detector 2x2 (default) or keep it at full resolution; drops existing coarse levels.
+        Wrappers returned earlier by coarsen() on this handle (and on its coarse levels) become unusable: call coarsen() again."""
+        self._drop_children()
         _check(load().cbct_set_detector_binning(self._h, 1 if on else 0))
 
     def device_bytes(self) -> int:
@@ -248,6 +264,7 @@ class Geometry:
 
     def close(self):
         if self._parent is None and getattr(self, "_h", None) is not None and self._h:
+            self._drop_children()         # cbct_geometry_destroy frees the coarse levels with the handle
             load().cbct_geometry_destroy(self._h)
         self._h = None
 

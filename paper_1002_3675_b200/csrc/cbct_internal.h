@@ -94,7 +94,9 @@ struct cbct_geometry {
     float *vol_a = nullptr, *vol_b = nullptr, *vol_c = nullptr, *vol_f = nullptr;   // g, u ping-pong, f
     float *Y_level = nullptr;                 // binned data for a coarse level
     float *vc_tau = nullptr, *vc_f0 = nullptr, *vc_d = nullptr, *vc_e = nullptr;   // V-cycle: tau, restricted iterate, gradient, scratch
-    float *fdk_q = nullptr, *fdk_hk = nullptr;   // FDK: pre-weighted, filtered projections; ramp taps D h[k], k odd
+    float *fdk_q = nullptr;                   // FDK: pre-weighted, filtered projections
+    double *fdk_hk = nullptr;                 // FDK: ramp taps D h[k], k odd
+    double2 *fdk_cs = nullptr;                // FDK: (cos, sin) of the views in fp64
     double *red_partial = nullptr;            // reduction partials
     double *red_out = nullptr;                // 2 doubles
     double *h_red = nullptr;                  // pinned host mirror of red_out

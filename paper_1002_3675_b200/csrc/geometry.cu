@@ -100,7 +100,7 @@ static void free_handle(cbct_geometry *g)
     free_handle(g->coarse);
     void *ptrs[] = {g->d_rays, g->d_rays_lo, g->d_zeta, g->d_inv_zeta, g->d_dz, g->d_cs, g->d_tiles[0], g->d_tiles[1],
                     g->d_angle_has[0], g->d_angle_has[1], g->vol_pad[0], g->vol_pad[1], g->proj_tmp, g->proj_prefix,
-                    g->G_cls[0], g->G_cls[1], g->vol_a, g->vol_b, g->vol_c, g->vol_f, g->Y_level, g->vc_tau, g->vc_f0, g->vc_d, g->vc_e, g->fdk_q, g->fdk_hk,
+                    g->G_cls[0], g->G_cls[1], g->vol_a, g->vol_b, g->vol_c, g->vol_f, g->Y_level, g->vc_tau, g->vc_f0, g->vc_d, g->vc_e, g->fdk_q, g->fdk_hk, g->fdk_cs,
                     g->red_partial, g->red_out, g->host_stage_vol, g->host_stage_proj, g->host_stage_vol2};
     for (void *p : ptrs) cbct_dev_free(g, p);
     if (g->h_red) cudaFreeHost(g->h_red);

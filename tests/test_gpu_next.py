@@ -100,6 +100,34 @@ def test_offset_cascade_and_full_resolution_detector(cuda_lib):
     G.close()
 
 
+def test_coarse_wrappers_do_not_outlive_their_level(cuda_lib):
+    """cbct_set_detector_binning and cbct_geometry_destroy free the coarse chain; the Python wrappers that pointed into it
+    must turn into clean errors (NULL handle), not dangling pointers."""
+    import torch
+    cb = cuda_lib
+    g = make_config("c3", shrink=8).geom
+    G = cb.Geometry.from_synth(g)
+    G1, _ = G.coarsen()
+    G2, _ = G1.coarsen()
+    v1 = torch.zeros(G1.vol_shape, device="cuda:0")
+    q1 = torch.empty(G1.proj_shape, device="cuda:0")
+    cb.forward(G1, v1, q1)                                   # usable while the level lives
+    G.set_detector_binning(False)                            # frees both coarse levels
+    assert G1._h is None and G2._h is None
+    for dead in (G1, G2):
+        with pytest.raises(cb.CbctError) as ei:
+            cb.forward(dead, torch.zeros(dead.vol_shape, device="cuda:0"), torch.empty(dead.proj_shape, device="cuda:0"))
+        assert ei.value.status == 1
+    H1, flags = G.coarsen()                                  # the level is rebuilt on demand, with the new choice
+    assert not flags[3] and (H1.nu, H1.nv) == (g.nu, g.nv)
+    cb.forward(H1, v1, torch.empty(H1.proj_shape, device="cuda:0"))
+    torch.cuda.synchronize()
+    G.close()
+    assert H1._h is None
+    with pytest.raises(cb.CbctError):
+        cb.forward(H1, v1, torch.empty(H1.proj_shape, device="cuda:0"))
+
+
 @pytest.mark.parametrize("case", ["c1_2_levels", "c3_shrunk_3_levels", "c4_shrunk_full_res_detector"])
 def test_fas_vcycles_match_the_oracle(cuda_lib, case):
     import torch
@@ -160,22 +188,52 @@ def test_fdk_matches_the_oracle(cuda_lib, case):
     # the filter alone on white noise (every tap matters): through the full call against the oracle
     Yn = f32(gaussian_field(g.proj_shape, 3))
     cb.fdk_reconstruct(G, to_dev(Yn), f)
-    assert rel(f.cpu().numpy(), o.fdk_reconstruct(g, Yn.astype(np.float64))) <= 5e-5
+    e = rel(f.cpu().numpy(), o.fdk_reconstruct(g, Yn.astype(np.float64)))
+    print(f"fdk {case} white-noise rel-L2 {e:.2e}")
+    assert e <= 1e-5
     G.close()
 
 
+def test_fdk_refuses_scans_its_weights_do_not_hold_for(cuda_lib):
+    """pi / N_theta per view is the quadrature of equally spaced views over a full turn (Q22): a 200-degree arc, a list with a
+    gap and a list with a doubled view return CBCT_ERR_SHAPE instead of a mis-scaled volume; a full turn run backwards or
+    started anywhere is accepted."""
+    import torch
+    cb = cuda_lib
+    base = dict(nu=48, nv=32, du=2.0, dv=2.0, nx=32, ny=32, nz=16, hx=1.5, hy=1.5, hz=2.0)
+    full = equispaced_angles(12)
+    bad = {"short scan": np.linspace(0.0, np.deg2rad(200.0), 12), "gap": np.delete(equispaced_angles(13), 5),
+           "doubled view": np.concatenate([full[:4], full[3:]])}
+    for name, ang in bad.items():
+        G = cb.Geometry.from_synth(Geometry(1000., 1500., ang, **base))
+        Y = torch.ones(G.proj_shape, device="cuda:0")
+        f = torch.empty(G.vol_shape, device="cuda:0")
+        with pytest.raises(cb.CbctError) as ei:
+            cb.fdk_reconstruct(G, Y, f)
+        assert ei.value.status == 2 and "equally spaced" in str(ei.value), name
+        G.close()
+    outs = []
+    for ang in (full, full[::-1].copy(), full + 0.7):
+        g = Geometry(1000., 1500., ang, **base)
+        G = cb.Geometry.from_synth(g)
+        Y = f32(gaussian_field(g.proj_shape, 5))
+        f = torch.empty(G.vol_shape, device="cuda:0")
+        cb.fdk_reconstruct(G, to_dev(Y), f)
+        assert rel(f.cpu().numpy(), o.fdk_reconstruct(g, Y.astype(np.float64))) <= 1e-5
+        G.close()
+
+
 def test_fdk_full_size_c3(cuda_lib):
-    """FDK at the full c3 size (512x512x64, 40 views of 512x384), every voxel.  Stated bound 3e-5: the
-    fp32 detector coordinate of a voxel, up to 256 pixels from the central ray, carries half an ulp = 1.5e-5 pixel, and the
-    ramp-filtered data change by their own size within a pixel at every edge; measured 1.2e-5 on the clean line integrals and on
-    the noisy data alike.  (The small cases above, with detectors of <= 150 pixels, meet 1e-5.)"""
+    """FDK at the full c3 size (512x512x64, 40 views of 512x384), every voxel, at the operator bound 1e-5 of north_star.  (Round 2
+    held this case to 3e-5 because the kernel placed voxels on the detector in fp32, half an ulp = 1.5e-5 pixel at 256 pixels
+    from the central ray; the positions are fp64 now and the bound is back where the small cases have it.)"""
     import torch
     cb = cuda_lib
     cfg = make_config("c3")
     g = cfg.geom
     G = cb.Geometry.from_synth(g)
     f = torch.empty(G.vol_shape, device="cuda:0")
-    for Y, tol in ((f32(cfg.clean_projections()), 3e-5), (f32(cfg.projections()), 3e-5)):
+    for Y, tol in ((f32(cfg.clean_projections()), 1e-5), (f32(cfg.projections()), 1e-5)):
         cb.fdk_reconstruct(G, to_dev(Y), f)
         ref = o.fdk_reconstruct(g, Y.astype(np.float64))
         e = rel(f.cpu().numpy(), ref)
