@@ -105,6 +105,12 @@ struct cbct_geometry {
     struct Guarded { void *ptr; size_t bytes, padded; };
     std::vector<Guarded> guarded;             // buffers allocated in guard mode (cbct_set_guard_mode): user pointer, sizes
 
+    // TV sweep (tv_tma.cu): encoded tensor maps of the volumes the sweeps read, keyed by (pointer, box); the dims are the
+    // handle's.  A map depends on nothing else, so an entry stays valid even if the caller frees and reuses the address.
+    struct TmapSlot { const void *ptr = nullptr; unsigned bx = 0, by = 0; alignas(64) unsigned char map[128]; };
+    TmapSlot tv_tmaps[8];
+    int tv_tmap_next = 0;                     // round-robin replacement
+
     int bp_parts = 1, G_parts_alloc[2] = {0, 0};   // gather: angle parts per column chunk (small volumes), partial volumes allocated
     int bp_mode = 0;                          // step 1 of A1: 0 exact transpose, 1 eq. 2 (cbct_set_backprojector)
     int use_mirror = 1;                        // march and gather: use the scan's mirror symmetry about z = 0 where it has one (cbct_set_mirror_symmetry)

@@ -14,6 +14,8 @@
 // store one 512-byte line group.  Per plane: fluxes of rows y0-1 .. y0+W-2 (qy to the row above through shared memory, one
 // barrier), then the update of rows y0 .. y0+W-2 with 16-byte stores.  HBM traffic per voxel and step: read u, read g,
 // write u' (12 B), each once (the halo rows of neighbouring CTAs come from L2).
+#include <mutex>
+
 #include "cbct_internal.h"
 #include "tma.cuh"
 
@@ -198,23 +200,61 @@ tv_tma_kernel(const __grid_constant__ CUtensorMap tm_u, const __grid_constant__ 
     }
 }
 
+// The tensor map of a volume of the handle's dims at `base` with a (bx, by, 1) box: from the handle's cache, else encoded
+// (about a microsecond of host time, which ten sweeps per outer iteration used to pay twice each) and remembered.
+// ok = false: the driver cannot encode (no cuTensorMapEncodeTiled) - the caller falls back to the row kernel.
+const CUtensorMap *tv_tensor_map(cbct_geometry *g, const float *base, unsigned bx, unsigned by, bool *ok)
+{
+    static_assert(sizeof(CUtensorMap) <= sizeof(cbct_geometry::TmapSlot::map), "TmapSlot::map holds a CUtensorMap");
+    *ok = true;
+    for (auto &s : g->tv_tmaps)
+        if (s.ptr == base && s.bx == bx && s.by == by) return reinterpret_cast<const CUtensorMap *>(s.map);
+    auto &s = g->tv_tmaps[g->tv_tmap_next];
+    g->tv_tmap_next = (g->tv_tmap_next + 1) % (int)(sizeof(g->tv_tmaps) / sizeof(g->tv_tmaps[0]));
+    const unsigned long long p1 = (unsigned long long)g->nx * sizeof(float), p2 = p1 * g->ny;
+    s.ptr = nullptr;
+    if (cbct_tensor_map_3d(reinterpret_cast<CUtensorMap *>(s.map), base, g->nx, g->ny, g->nz, p1, p2, bx, by, 1) != CBCT_OK) {
+        *ok = false;
+        return nullptr;
+    }
+    s.ptr = base; s.bx = bx; s.by = by;
+    return reinterpret_cast<const CUtensorMap *>(s.map);
+}
+
+// *launched = false (and CBCT_OK) if the tensor maps cannot be encoded: nothing has been launched, the caller uses tv_rows.cu.
 template <int CH, int W>
 cbct_status launch_tma(cbct_geometry *g, const float *u_in, const float *gv, float *u_out, float beta, float eps, float dt,
-                       int clamp, cudaStream_t st)
+                       int clamp, cudaStream_t st, bool *launched)
 {
     using L = TvTmaLayout<CH, W>;
     auto kern = tv_tma_kernel<CH, W>;
     const size_t smem = L::total(g->nx);
-    static int slots = 0;
+    *launched = false;
+    const unsigned bx = (unsigned)L::bx(g->nx);
+    bool ok = true;
+    const CUtensorMap *pu = tv_tensor_map(g, u_in, bx, W + 1, &ok);
+    // with g fetched by plain 16-byte loads (kGLdg) the kernel never touches its second map: the first one fills the slot
+    const CUtensorMap *pg = (ok && !kGLdg) ? tv_tensor_map(g, gv, bx, W - 1, &ok) : pu;
+    if (!ok) return CBCT_OK;
+    const CUtensorMap tu = *pu, tg = *pg;
+    // kernel attribute and occupancy, cached per instantiation for the whole process; handles may live on different host
+    // threads (cbct.h: one handle per thread), so the cache is read and written under a lock
+    static std::mutex mtx;
+    static int slots_cached = 0;
     static size_t smem_set = 0;
-    if (!slots || smem > smem_set) {
-        CBCT_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        int dev = 0, sms = 0, per_sm = 0;
-        CBCT_CUDA(cudaGetDevice(&dev));
-        CBCT_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-        CBCT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 32 * W, smem));
-        slots = sms * (per_sm > 0 ? per_sm : 1);
-        smem_set = smem;
+    int slots;
+    {
+        std::lock_guard<std::mutex> lock(mtx);
+        if (!slots_cached || smem > smem_set) {
+            CBCT_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            int dev = 0, sms = 0, per_sm = 0;
+            CBCT_CUDA(cudaGetDevice(&dev));
+            CBCT_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+            CBCT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 32 * W, smem));
+            slots_cached = sms * (per_sm > 0 ? per_sm : 1);
+            smem_set = smem;
+        }
+        slots = slots_cached;
     }
     const int ytiles = (g->ny + W - 2) / (W - 1);
     int zchunk = 8;
@@ -224,16 +264,12 @@ cbct_status launch_tma(cbct_geometry *g, const float *u_in, const float *gv, flo
         const long cost = ((ctas + slots - 1) / slots) * (zc + 1);
         if (best < 0 || cost < best) { best = cost; zchunk = zc; }
     }
-    CUtensorMap tu, tg;
-    const unsigned long long p1 = (unsigned long long)g->nx * sizeof(float), p2 = p1 * g->ny;
-    const unsigned bx = (unsigned)L::bx(g->nx);
-    CBCT_TRY(cbct_tensor_map_3d(&tu, u_in, g->nx, g->ny, g->nz, p1, p2, bx, W + 1, 1));
-    CBCT_TRY(cbct_tensor_map_3d(&tg, gv, g->nx, g->ny, g->nz, p1, p2, bx, W - 1, 1));
     const double hx = g->hx, hy = g->hy, hz = g->hz;
     dim3 grid(ytiles, (g->nz + zchunk - 1) / zchunk);
     kern<<<grid, 32 * W, smem, st>>>(tu, tg, gv, u_out, g->nx, g->ny, g->nz, (float)(1.0 / (hx * hx)), (float)(1.0 / (hy * hy)),
                                      (float)(1.0 / (hz * hz)), beta, eps * eps, dt, clamp ? 0.f : -INFINITY, zchunk);
     CBCT_LAUNCH_CHECK();
+    *launched = true;
     return CBCT_OK;
 }
 }  // namespace
@@ -242,17 +278,21 @@ cbct_status launch_tma(cbct_geometry *g, const float *u_in, const float *gv, flo
 #define CBCT_TV_TMA_W 8
 #endif
 
-// *done = 1 if this path took the step (nx <= 512, nx % 4 == 0, 16-byte aligned volumes, at least 32 voxels per row).
+// *done = 1 if this path took the step (nx <= 512, nx % 4 == 0, 16-byte aligned volumes, at least 32 voxels per row, and a
+// driver that encodes tensor maps); *done = 0 with CBCT_OK means nothing was launched and the caller takes the row kernel.
 cbct_status op_tv_sweep_tma(cbct_geometry *g, const float *u_in, const float *gv, float *u_out, float beta, float eps, float dt,
                             int clamp, cudaStream_t st, int *done)
 {
     *done = 0;
     const int nx = g->nx;
     if (nx > 512 || nx < 32 || nx % 4 != 0 || (((uintptr_t)u_in | (uintptr_t)gv | (uintptr_t)u_out) & 15) != 0) return CBCT_OK;
-    *done = 1;
     constexpr int W = CBCT_TV_TMA_W;
-    if (nx <= 128) return launch_tma<1, W>(g, u_in, gv, u_out, beta, eps, dt, clamp, st);
-    if (nx <= 256) return launch_tma<2, W>(g, u_in, gv, u_out, beta, eps, dt, clamp, st);
-    if (nx <= 384) return launch_tma<3, W>(g, u_in, gv, u_out, beta, eps, dt, clamp, st);
-    return launch_tma<4, W>(g, u_in, gv, u_out, beta, eps, dt, clamp, st);
+    bool launched = false;
+    cbct_status rc;
+    if (nx <= 128) rc = launch_tma<1, W>(g, u_in, gv, u_out, beta, eps, dt, clamp, st, &launched);
+    else if (nx <= 256) rc = launch_tma<2, W>(g, u_in, gv, u_out, beta, eps, dt, clamp, st, &launched);
+    else if (nx <= 384) rc = launch_tma<3, W>(g, u_in, gv, u_out, beta, eps, dt, clamp, st, &launched);
+    else rc = launch_tma<4, W>(g, u_in, gv, u_out, beta, eps, dt, clamp, st, &launched);
+    *done = launched ? 1 : 0;
+    return rc;
 }
