@@ -37,6 +37,34 @@ def test_lambda_max_power_iteration():
     assert o.lambda_max(g, iters=60) == pytest.approx(lam, rel=1e-3)
 
 
+def test_step1_is_the_papers_update_with_its_constant():
+    """P:87 verbatim: g = f - (mu V / beta) dE2/df.  On the grid V = N_vox dV and the functional derivative is (1/dV) times
+    the partial derivative with respect to a voxel value, so the update is g = f - (mu N_vox / beta) grad E2(f).  One outer
+    iteration without TV steps and without the clamp returns g itself; grad E2 comes from central differences of the
+    separately evaluated energy term (E2 is quadratic in f, so they are exact up to rounding) at EVERY voxel.  This pins the
+    constant c = 2 step N_vox / (N_theta N_pix) of fbs_level, factor 2 included, against eq. 1's E2."""
+    g = toy()
+    _, f_true, Y = toy_data(g, seed=3)
+    rng = np.random.default_rng(5)
+    f0 = f_true + 0.01 * rng.random(g.vol_shape)
+    mu, step, eps = 3.0, 0.37, 1e-3
+    beta = mu / step
+    f1 = fbs.fbs_level(g, Y, f0, 1, 0, step, mu, eps, clamp=False)
+    E2 = lambda f: fbs.energy(g, f, Y, mu, eps)["E2"]
+    grad = np.zeros(g.vol_shape)
+    d = 1e-2
+    for idx in np.ndindex(*g.vol_shape):
+        fp, fm = f0.copy(), f0.copy()
+        fp[idx] += d
+        fm[idx] -= d
+        grad[idx] = (E2(fp) - E2(fm)) / (2 * d)
+    lhs, rhs = (f0 - f1) * beta, g.n_vox * mu * grad
+    assert np.abs(rhs).max() > 0
+    assert np.abs(lhs - rhs).max() <= 1e-9 * np.abs(rhs).max()
+    # a dropped factor 2, N_vox or 1/(N_theta N_pix) would be off by far more than this
+    assert np.abs(lhs - 0.5 * rhs).max() > 0.1 * np.abs(rhs).max()
+
+
 @pytest.mark.parametrize("u0_mode,clamp", [("g", True), ("f", False)])
 def test_I10_dense_matrix_fbs(u0_mode, clamp):
     """O5 = Algorithm A1 with explicit numpy matrix algebra, per iteration."""
