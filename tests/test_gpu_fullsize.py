@@ -67,6 +67,38 @@ def test_c2_operator_bench_config(cuda_lib):
     assert e_fwd <= 1e-5 and e_bp <= 1e-5 and e_adj <= 1e-5, (e_fwd, e_bp, e_adj)
 
 
+def maxerr(a, b):
+    a = np.asarray(a, dtype=np.float64)
+    return float(np.abs(a - b).max() / max(np.abs(b).max(), 1e-300))
+
+
+def test_c2_every_ray_and_every_voxel(cuda_lib):
+    """The benchmarked config in full, not a sample: all 7.86 M rays of P(phantom) and all 16.8 M voxels of P^T(P(phantom))
+    against the oracle (about 20 s of oracle time on 16 cores), rel-L2 <= 1e-5 and every element within 1e-4 of the largest
+    (K_MAX * TOL_OP of tests/test_gpu_parity.py), in the launch configuration bench.py times (default kernels)."""
+    import torch
+    cb = cuda_lib
+    dev = torch.device("cuda:0")
+    cfg = make_config("c2")
+    g = cfg.geom
+    G = cb.Geometry.from_synth(g)
+    vol = f32(cfg.volume())
+    d_q = torch.empty(g.proj_shape, device=dev)
+    d_b = torch.empty(g.vol_shape, device=dev)
+    cb.forward(G, torch.from_numpy(vol).to(dev), d_q)
+    cb.backproject(G, d_q, d_b)
+    q, b = d_q.cpu().numpy(), d_b.cpu().numpy()
+    G.close()
+    q_ref = o.forward(g, vol.astype(np.float64))
+    b_ref = o.backproject(g, q.astype(np.float64))
+    print(f"PARITY c2 whole arrays: P {rel(q, q_ref):.2e} / max {maxerr(q, q_ref):.2e}   Pt {rel(b, b_ref):.2e} / max {maxerr(b, b_ref):.2e}")
+    assert np.linalg.norm(q_ref) > 0 and np.linalg.norm(b_ref) > 0
+    assert rel(q, q_ref) <= 1e-5 and maxerr(q, q_ref) <= 1e-4
+    assert rel(b, b_ref) <= 1e-5 and maxerr(b, b_ref) <= 1e-4
+    # rays that miss the volume: exactly where the oracle has zeros, up to grazing rays (a few 1e-7 of a voxel)
+    assert np.all(np.abs(q[q_ref == 0.0]) <= 1e-6 * np.abs(q_ref).max())
+
+
 @pytest.mark.parametrize("name", ["c3", "c4"])
 def test_c3_c4_operators_full_size(cuda_lib, name):
     e_fwd, e_bp, e_adj = sampled_operator_parity(cuda_lib, make_config(name))

@@ -26,6 +26,19 @@ def rel(a, b):
     return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
 
 
+def maxerr(a, b):
+    """Largest element error over the largest element of the oracle's array (the per-element companion of rel)."""
+    a = np.asarray(a, dtype=np.float64)
+    return float(np.abs(a - b).max() / max(np.abs(b).max(), 1e-300))
+
+
+# Per-element bound beside every operator rel-L2: max|gpu - oracle| <= K_MAX * TOL_OP * max|oracle|.  rel-L2 at 1e-5 sees one
+# element that is 10 % off among 1e7 but not one that is 1 % off; this bound does (K_MAX * TOL_OP = 1e-4 of the largest
+# element).  K_MAX = 10: fp32 sums of a few hundred chord * value products carry element errors of a few 1e-7 of the largest
+# element on smooth inputs and up to ~5e-6 on Gaussian ones (printed by the tests, recorded in DESIGN.md "Tolerances").
+K_MAX = 10.0
+
+
 @pytest.fixture(scope="module")
 def dev(cuda_lib):
     import torch
@@ -98,13 +111,13 @@ def test_forward_backproject_adjoint(cuda_lib, dev, name):
     vol = f32(smooth_phantom(g, 3) if name != "c1" else make_config("c1").volume())
     q = run_forward(cb, G, vol, dev)
     q_ref = o.forward(g, vol.astype(np.float64))
-    assert rel(q, q_ref) <= TOL_OP
+    assert rel(q, q_ref) <= TOL_OP and maxerr(q, q_ref) <= K_MAX * TOL_OP
     # rays that miss the volume give 0 (a ray grazing an edge within fp32 rounding may leave ~1e-7 of a voxel)
     assert np.all(np.abs(q[q_ref == 0.0]) <= 1e-6 * np.abs(q_ref).max())
     assert np.count_nonzero(q[q_ref == 0.0]) <= 0.01 * max(1, np.count_nonzero(q_ref == 0.0))
     b = run_backproject(cb, G, q, dev)                         # backproject on P(phantom)
     b_ref = o.backproject(g, q.astype(np.float64))
-    assert rel(b, b_ref) <= TOL_OP
+    assert rel(b, b_ref) <= TOL_OP and maxerr(b, b_ref) <= K_MAX * TOL_OP
     # adjoint identity on seeded Gaussian x, y (dot products in fp64)
     x = f32(gaussian_field(g.vol_shape, 11))
     y = f32(gaussian_field(g.proj_shape, 12))
@@ -112,9 +125,18 @@ def test_forward_backproject_adjoint(cuda_lib, dev, name):
     Pty = run_backproject(cb, G, y, dev).astype(np.float64)
     lhs, rhs = np.vdot(Px, y.astype(np.float64)), np.vdot(x.astype(np.float64), Pty)
     assert abs(lhs - rhs) / (np.linalg.norm(Px) * np.linalg.norm(y)) <= TOL_ADJ
-    # Gaussian inputs are the worst case for fp32 chord boundaries: stated bound 5e-5
-    assert rel(Px, o.forward(g, x.astype(np.float64))) <= 5e-5
-    assert rel(Pty, o.backproject(g, y.astype(np.float64))) <= 5e-5
+    # Gaussian inputs are the worst case for fp32 chord boundaries (no smoothness to average the boundary errors out)
+    Px_ref, Pty_ref = o.forward(g, x.astype(np.float64)), o.backproject(g, y.astype(np.float64))
+    print(f"PARITY {name}: P phantom {rel(q, q_ref):.1e}/{maxerr(q, q_ref):.1e}  Pt {rel(b, b_ref):.1e}/{maxerr(b, b_ref):.1e}  "
+          f"P gauss {rel(Px, Px_ref):.1e}/{maxerr(Px, Px_ref):.1e}  Pt gauss {rel(Pty, Pty_ref):.1e}/{maxerr(Pty, Pty_ref):.1e}")
+    # The gather places its crossings with two-float positions and holds the operator bound on white noise as well (measured
+    # 6e-8 .. 5e-7).  The march reads fp32 ray tables: a chord boundary sits up to ~3e-5 voxel off, which smooth volumes
+    # average out (1e-7 .. 2.5e-6 above) and white noise does not: measured 5e-7 .. 8e-6, 2.8e-5 on the one-column detector
+    # (no neighbouring columns to share a boundary error with).  Stated bound for the march on white noise: 5e-5 (DESIGN.md
+    # "Tolerances"; SURVEY.md section 7 anticipated it).
+    TOL_MARCH_NOISE = 5e-5
+    assert rel(Px, Px_ref) <= TOL_MARCH_NOISE and maxerr(Px, Px_ref) <= K_MAX * TOL_MARCH_NOISE
+    assert rel(Pty, Pty_ref) <= TOL_OP and maxerr(Pty, Pty_ref) <= K_MAX * TOL_OP
     G.close()
 
 
@@ -170,13 +192,14 @@ def test_plain_kernels_equal_the_mirrored_kernels(cuda_lib, dev, name):
     # of the same ray): equal to a few 1e-7
     assert rel(q_m, q_p.astype(np.float64)) <= 0.5 * TOL_OP
     assert rel(q_m, o.forward(g, vol.astype(np.float64))) <= TOL_OP
-    for y, tol in ((q_m, TOL_OP), (f32(gaussian_field(g.proj_shape, 21)), 5e-5)):
+    for y, tol in ((q_m, TOL_OP), (f32(gaussian_field(g.proj_shape, 21)), TOL_OP)):
         ref = o.backproject(g, y.astype(np.float64))
         G.set_mirror_symmetry(True)
         b_m = run_backproject(cb, G, y, dev)
         G.set_mirror_symmetry(False)
         b_p = run_backproject(cb, G, y, dev)
         assert rel(b_m, ref) <= tol and rel(b_p, ref) <= tol
+        assert maxerr(b_m, ref) <= K_MAX * tol and maxerr(b_p, ref) <= K_MAX * tol
         assert rel(b_m, b_p.astype(np.float64)) <= 0.2 * tol          # both are one matrix: far closer to each other than to the bound
     # the loop (residual modes of the march, gradient step) agrees too
     Y = to_dev(0.9 * q_m + 0.01, dev)
