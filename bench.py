@@ -245,24 +245,16 @@ def run_gpu(args):
     nnz_fine = float(frozen("nnz", "c2", NNZ["c2"]))
     nnz_step = nnz_fine * (1.0 + frozen("nnz_coarse_ratio", "c2", 0.125))
     sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
-    traffic = None                      # DRAM bytes per launch of that kernel from the committed ncu capture (profiles/traffic.csv)
-    try:
-        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as fh:
-            for line in fh.read().splitlines()[1:]:
-                k, v = line.split(",")[:2]
-                if k == dom:
-                    traffic = float(v)
-    except Exception:
-        pass
+    traffic, traffic_stale = committed_traffic(dom)
     if dom == "tv_sweep":
         roof = {"kernel": "tv_sweep_kernel", "bound": "hbm", "achieved": tv_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s",
-                "frac": tv_gbs / pk["hbm_gbs"], "traffic": traffic, "traffic_covers": TRAFFIC_COVERS,
+                "frac": tv_gbs / pk["hbm_gbs"], "traffic": traffic, "traffic_stale": traffic_stale, "traffic_covers": TRAFFIC_COVERS,
                 "peak_source": "MEASURED_PEAKS.json copy bandwidth" if pk["which"] == "measured" else "fallback (B200_PROFILING.md)"}
     else:
         peak = sm_count * 128 * pk["sm_max_mhz"] * 1e6 / 1e12            # T lane-op/s (fp32 issue: SMs x 128 lanes x clock)
         ach = LANE_OPS_PER_CHORD * nnz_step / (per_step_ms(dom) / 1e3) / 1e12
         roof = {"kernel": dom + "_kernel", "bound": "alu", "achieved": ach, "peak": peak, "unit": "Tlane-op/s",
-                "frac": ach / peak, "traffic": traffic, "traffic_covers": TRAFFIC_COVERS,
+                "frac": ach / peak, "traffic": traffic, "traffic_stale": traffic_stale, "traffic_covers": TRAFFIC_COVERS,
                 "peak_source": f"nominal lanes ({sm_count} SMs x 128 fp32 lanes) x max SM clock ({pk['sm_max_mhz']:.0f} MHz, {pk['which']})",
                 "model": f"{LANE_OPS_PER_CHORD} fp32 lane-ops per chord x {nnz_step:.3e} chords per step (SURVEY.md 8(d))",
                 "chords_per_s": nnz_step / (per_step_ms(dom) / 1e3)}
@@ -293,6 +285,17 @@ def run_gpu(args):
         extra["gups_backproject_eq2"] = g.n_vox * g.n_angles / (ea.elapsed_time(eb) / 5e3) / 1e9
         # NEXT-4 (not part of `value`): the FDK baseline on c3's data, beside the FBS reconstruction of the same scan
         extra["sec_fdk_c3"] = time_c3_fdk(cb, dev, st)
+        # metric (3) of BASELINE.json on the other configs, and the c3 reconstruction end to end from host buffers
+        extra["sec_per_fbs_recon_c1"] = time_recon(cb, dev, st, "c1")
+        extra["sec_per_fbs_recon_c4"] = time_recon(cb, dev, st, "c4")
+        sec_h, h2d, d2h = time_c3_recon_host(cb, dev, st)
+        extra["sec_per_fbs_recon_c3_e2e_host"] = {"value": sec_h, "h2d_bytes": h2d, "d2h_bytes": d2h,
+                                                  "through": "cbct_fbs_reconstruct_host, pinned host buffers, host clock"}
+        if not args.no_c5:
+            sec5, (gp5, gb5) = time_recon(cb, dev, st, "c5", synthetic_noise_only=True, operators=True)
+            extra.update(sec_per_fbs_recon_c5=sec5, gups_forward_c5=gp5, gups_backproject_c5=gb5,
+                         c5_note="512^3 volume, 363 views of 1024 x 768, 3 levels x 50 outer x 10 TV sweeps; projections are "
+                                 "device-made uniform noise (fixed iteration counts: the work does not depend on the values)")
     cpu = cpu_baseline_sample(cfg, n_angles=args.cpu_angles) if world == 1 and not args.no_cpu else None
 
     line = {
@@ -376,13 +379,50 @@ def run_sharded(args):
         dist.destroy_process_group()
 
 
-def time_c3_recon(cb, dev, st, eq2=False):
-    """seconds per full c3 reconstruction (2 levels x 100 outer x 10 inner; noisy 40-view data)."""
+def kernel_source_sha(rel_path):
+    """First 16 hex digits of the SHA-256 of a kernel source file (the stamp profiles/traffic.csv carries per row)."""
+    import hashlib
+    with open(os.path.join(ROOT, rel_path), "rb") as fh:
+        return hashlib.sha256(fh.read()).hexdigest()[:16]
+
+
+def committed_traffic(kernel_class):
+    """(DRAM bytes per launch of that kernel class from the committed ncu capture, None) - or (None, reason) when
+    profiles/traffic.csv has no row for the class or its row was captured from ANOTHER version of the kernel's source file:
+    a traffic figure that no longer belongs to the kernel being timed is reported as missing, loudly, not carried along.
+    Rows: kernel_class,dram_bytes_per_launch,source_file,source_sha256_16,capture."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as fh:
+            rows = [line.split(",", 4) for line in fh.read().splitlines()[1:] if line.strip()]
+    except OSError as e:
+        return None, f"profiles/traffic.csv: {e}"
+    for r in rows:
+        if r[0] == kernel_class:
+            if len(r) < 4:
+                return None, "profiles/traffic.csv row carries no source stamp"
+            now = kernel_source_sha(r[2])
+            if now != r[3]:
+                return None, (f"{r[2]} has changed since the ncu capture in profiles/traffic.csv (stamp {r[3]}, now {now}): "
+                              "re-capture with ncu --set full and update the row")
+            return float(r[1]), None
+    return None, f"profiles/traffic.csv has no row for {kernel_class}"
+
+
+def time_recon(cb, dev, st, name, eq2=False, synthetic_noise_only=False, operators=False):
+    """Seconds per full reconstruction of config `name` at its own level and iteration counts (c1: 1 x 20 outer x 5 inner;
+    c3 / c4: 2 / 3 levels x 100 x 10; c5: 3 levels x 50 x 10), device-resident data, CUDA events on the launching stream, after
+    a short warm-up cascade that makes every allocation.  synthetic_noise_only (c5): the 363 projections of 1024 x 768 are
+    uniform noise made on the device instead of line integrals of the phantom (a minute of host time saved; with fixed
+    iteration counts the kernels' work does not depend on the values).  operators: also returns projector / backprojector GUPS
+    at that size (mean of 2 applications each)."""
     import torch
     from cbct_synth import make_config
-    cfg = make_config("c3")
+    cfg = make_config(name)
     g = cfg.geom
-    Y = torch.from_numpy(np.ascontiguousarray(cfg.projections(), dtype=np.float32)).to(dev)
+    if synthetic_noise_only:
+        Y = torch.rand(g.proj_shape, device=dev) * 20.0
+    else:
+        Y = torch.from_numpy(np.ascontiguousarray(cfg.projections(), dtype=np.float32)).to(dev)
     G = cb.Geometry.from_synth(g)
     if eq2:
         cb.set_backprojector(G, cb.BACKPROJECTOR_EQ2)
@@ -394,8 +434,52 @@ def time_c3_recon(cb, dev, st, eq2=False):
         cb.fbs_reconstruct(G, Y, None, cfg.n_levels, cfg.n_outer, cfg.n_inner, cfg.step, cfg.mu, cfg.eps, cfg.omega, f, stream=st)
         b.record(st)
     torch.cuda.synchronize()
+    sec = a.elapsed_time(b) / 1e3
+    ops = None
+    if operators:
+        q = torch.empty(g.proj_shape, device=dev)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        with torch.cuda.stream(st):
+            cb.forward(G, f, q, stream=st)
+            cb.backproject(G, q, f, stream=st)
+            ev[0].record(st)
+            for _ in range(2):
+                cb.forward(G, f, q, stream=st)
+            ev[1].record(st)
+            for _ in range(2):
+                cb.backproject(G, q, f, stream=st)
+            ev[2].record(st)
+        torch.cuda.synchronize()
+        upd = float(g.n_vox) * g.n_angles
+        ops = (upd / (ev[0].elapsed_time(ev[1]) / 2e3) / 1e9, upd / (ev[1].elapsed_time(ev[2]) / 2e3) / 1e9)
     G.close()
-    return a.elapsed_time(b) / 1e3
+    return (sec, ops) if operators else sec
+
+
+def time_c3_recon(cb, dev, st, eq2=False):
+    """seconds per full c3 reconstruction (2 levels x 100 outer x 10 inner; noisy 40-view data)."""
+    return time_recon(cb, dev, st, "c3", eq2=eq2)
+
+
+def time_c3_recon_host(cb, dev, st):
+    """Seconds per full c3 reconstruction END TO END through cbct_fbs_reconstruct_host, the call a user with host data makes:
+    pinned host buffers, the upload of Y (31.5 MB) and the download of f (67 MB) inside the timed region, host clock around the
+    call (it returns after synchronising its stream); second of two calls (the first makes the allocations)."""
+    import torch
+    from cbct_synth import make_config
+    cfg = make_config("c3")
+    g = cfg.geom
+    h_Y = torch.from_numpy(np.ascontiguousarray(cfg.projections(), dtype=np.float32)).pin_memory()
+    h_f = torch.empty(g.vol_shape, dtype=torch.float32).pin_memory()
+    G = cb.Geometry.from_synth(g)
+    args = (cfg.n_inner, cfg.step, cfg.mu, cfg.eps, cfg.omega)
+    cb.fbs_reconstruct_host(G, h_Y, None, cfg.n_levels, [2] * cfg.n_levels, *args, h_f, stream=st)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    cb.fbs_reconstruct_host(G, h_Y, None, cfg.n_levels, cfg.n_outer, *args, h_f, stream=st)
+    sec = time.perf_counter() - t0
+    G.close()
+    return sec, int(h_Y.numel() * 4), int(h_f.numel() * 4)
 
 
 def time_tv_512(cb, dev, st, flush):
@@ -466,6 +550,46 @@ def cpu_baseline_sample(cfg, n_angles=8, steps=1, warmup=0):
                       f"views of c2 at full 256^3 volume size, fp64, OpenMP"}
 
 
+def run_ops_only(args):
+    """--ops-only NAME: one projection, one exact backprojection and one TV sweep at the size of config NAME (plus one TV sweep
+    on a 512^3 volume for c5), after one untimed application of each, and nothing else.  Not a bench line: this is the
+    command the ncu captures at sizes that leave L2 are taken from (profiles/r03_*); it prints the three event times."""
+    import torch
+    import paper_1002_3675_b200 as cb
+    from cbct_synth import make_config
+    dev = torch.device("cuda:0")
+    torch.cuda.set_device(dev)
+    g = make_config(args.ops_only).geom
+    G = cb.Geometry.from_synth(g)
+    f = torch.rand(g.vol_shape, device=dev) * 0.02
+    u = f.clone()
+    q = torch.empty(g.proj_shape, device=dev)
+    b = torch.empty(g.vol_shape, device=dev)
+    st = torch.cuda.Stream()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    with torch.cuda.stream(st):
+        for timed in (False, True):
+            if timed:
+                ev[0].record(st)
+            cb.forward(G, f, q, stream=st)
+            if timed:
+                ev[1].record(st)
+            cb.backproject(G, q, b, stream=st)
+            if timed:
+                ev[2].record(st)
+            cb.tv_prox(G, f, u, 4.0e4, 1e-4, 1.0, 1, stream=st)
+            if timed:
+                ev[3].record(st)
+    torch.cuda.synchronize()
+    ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(3)]
+    upd = float(g.n_vox) * g.n_angles
+    print(json.dumps({"ops_only": args.ops_only, "dims": [g.nx, g.ny, g.nz, g.n_angles, g.nu, g.nv],
+                      "ms_forward": ms[0], "ms_backproject": ms[1], "ms_tv_sweep": ms[2],
+                      "gups_forward": upd / ms[0] / 1e6, "gups_backproject": upd / ms[1] / 1e6,
+                      "tv_GBps": 12.0 * g.n_vox / ms[2] / 1e6}))
+    G.close()
+
+
 def run_reference(args):
     """--impl reference: the oracle, as it stands, on the host cores; each step a bounded sample."""
     rank = int(os.environ.get("RANK", "0"))
@@ -511,6 +635,9 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
     ap.add_argument("--no-recon", action="store_true", help="skip the full c3 reconstruction timing")
+    ap.add_argument("--no-c5", action="store_true", help="skip the c5 (512^3, 363 views) reconstruction and operator timing (~30 s)")
+    ap.add_argument("--ops-only", default="", metavar="CONFIG",
+                    help="one projection, backprojection and TV sweep at the size of a config (c2..c5) and exit: the ncu target of profiles/r03_*")
     ap.add_argument("--cpu-angles", type=int, default=8)
     ap.add_argument("--shard-angles", action="store_true",
                     help="NEXT-4: shard the views of ONE reconstruction over the ranks (strong scaling) instead of replicas")
@@ -532,6 +659,8 @@ def main():
         run_reference(args)
     elif args.shard_angles:
         run_sharded(args)
+    elif args.ops_only:
+        run_ops_only(args)
     else:
         run_gpu(args)
 
